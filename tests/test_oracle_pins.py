@@ -1,0 +1,444 @@
+"""Pins for the oracle (`-m "not gpu"`): the oracle is checked against what the paper and the
+mathematics fix — never against itself and never against the CUDA path.  Pin numbers follow
+SURVEY.md §8(c) / DESIGN.md §5."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import gp_workloads as W
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+# ------------------------------------------------------------------ independent numpy helpers
+def np_rho(kind, r, ell):
+    """The three closed-form correlation functions of BASELINE.json, written independently in numpy."""
+    if kind == "se":
+        return np.exp(-0.5 * (r / ell) ** 2)
+    if kind == "matern32":
+        a = math.sqrt(3.0) * r / ell
+        return (1.0 + a) * np.exp(-a)
+    if kind == "exp":
+        return np.exp(-r / ell)
+    raise ValueError(kind)
+
+
+def np_dense_K(x, kind, sigma, ell, jitter):
+    diff = x[:, None, :] - x[None, :, :]
+    r = np.sqrt((diff * diff).sum(-1))
+    K = sigma ** 2 * np_rho(kind, r, ell)
+    K[np.diag_indices_from(K)] = sigma ** 2 * (1.0 + jitter)
+    return K
+
+
+def rel(a, b):
+    return np.max(np.abs(np.asarray(a) - np.asarray(b))) / np.max(np.abs(b))
+
+
+KERNELS = [("se", 1.3, 0.2, 1e-6), ("matern32", 0.7, 0.15, 1e-6), ("exp", 1.1, 0.3, 0.0)]
+
+
+# ------------------------------------------------------------------ P-1 dense equivalence
+@pytest.mark.parametrize("kind,sigma,ell,jit", KERNELS)
+def test_p1_all_preceding_equals_dense_cholesky(orc, kind, sigma, ell, jit):
+    """c(i) = all preceding points  =>  v = L xi with K = L L^T (LAPACK), logdet = log det K.
+    BASELINE config 1's cross-check: N = 256, k = N - 1."""
+    n = 256
+    x = W.make_points(W.CONFIGS[1], "f64", n)
+    xi = W.make_noise(1, n, "f64")
+    kern = orc.Kernel(kind, sigma, ell, jit)
+    K = np_dense_K(x, kind, sigma, ell, jit)
+    L = np.linalg.cholesky(K)
+    v_dense = L @ xi
+    rowptr, col = orc.all_preceding_csr(n)
+    v = orc.forward(x, kern, xi, rowptr=rowptr, col=col)
+    assert rel(v, v_dense) < 1e-12
+    ld = orc.logdet(x, kern, rowptr=rowptr, col=col)
+    sign, ld_dense = np.linalg.slogdet(K)
+    assert sign > 0 and abs(ld - ld_dense) / abs(ld_dense) < 1e-12
+    xi_back = orc.inverse(x, kern, v_dense, rowptr=rowptr, col=col)
+    assert rel(xi_back, xi) < 1e-9
+    # the regular-graph driver with n0 = N (Alg. 1 line 1 only) is the same thing
+    v_head = orc.forward(x, kern, xi, n0=n, k=8, nbr=np.zeros((0, 8), np.int32))
+    assert rel(v_head, v_dense) < 1e-12
+    ld_head = orc.logdet(x, kern, n0=n, k=8, nbr=np.zeros((0, 8), np.int32))
+    assert abs(ld_head - ld_dense) / abs(ld_dense) < 1e-12
+
+
+def test_p1_regular_head_plus_rows_equals_ragged(orc):
+    """Alg. 1 line 1 (dense head) + per-point rows == every point through Eq. 2 with c(i)={0..i-1} for i<n0."""
+    cfg = W.CONFIGS[1]
+    n, n0, k = 600, 64, 8
+    x = W.make_points(cfg, "f64", n)
+    g = orc.build_graph(x, k, n0)
+    kern = orc.Kernel("se", 1.0, 0.1, 1e-6)
+    xi = W.make_noise(1, n, "f64")
+    rp = [0]
+    cols = []
+    for i in range(n):
+        c = np.arange(i, dtype=np.int32) if i < n0 else g.nbr[i - n0]
+        cols.append(c)
+        rp.append(rp[-1] + c.size)
+    rowptr, col = np.array(rp, np.int64), np.concatenate(cols).astype(np.int32)
+    v_reg = orc.forward(g.x, kern, xi, n0=n0, k=k, nbr=g.nbr, batch_off=g.batch_off)
+    v_rag = orc.forward(g.x, kern, xi, rowptr=rowptr, col=col)
+    assert rel(v_reg, v_rag) < 1e-11
+    vbar = W.make_noise(1, n, "f64", "vbar")
+    xb1, tb1 = orc.vjp(g.x, kern, xi, v_reg, vbar, n0=n0, k=k, nbr=g.nbr, batch_off=g.batch_off)
+    xb2, tb2 = orc.vjp(g.x, kern, xi, v_rag, vbar, rowptr=rowptr, col=col)
+    # dense-head VJP by the Cholesky-derivative formula == per-point closed forms (two different routes)
+    assert rel(xb1, xb2) < 1e-9
+    assert np.all(np.abs(tb1 - tb2) / np.abs(tb2) < 1e-8)
+    l1, g1 = orc.logdet(g.x, kern, n0=n0, k=k, nbr=g.nbr, grad=True)
+    l2, g2 = orc.logdet(g.x, kern, rowptr=rowptr, col=col, grad=True)
+    assert abs(l1 - l2) / abs(l2) < 1e-12
+    assert np.all(np.abs(g1 - g2) / np.abs(g2) < 1e-8)
+
+
+# ------------------------------------------------------------------ P-2 inverse o forward = id
+@pytest.mark.parametrize("cid,n", [(1, 4096), (2, 8192), (3, 8192), (4, 8192)])
+def test_p2_inverse_of_forward_is_identity(orc, cid, n):
+    cfg = W.CONFIGS[cid]
+    x = W.make_points(cfg, "f64", n)
+    g = orc.build_graph(x, cfg.k, min(cfg.n0, 256))
+    kern = orc.Kernel(cfg.kind, cfg.sigma, cfg.ell, cfg.jitter)
+    xi = W.make_noise(cid, n, "f64")
+    v = orc.forward(g.x, kern, xi, n0=g.n0, k=g.k, nbr=g.nbr, batch_off=g.batch_off)
+    xi2 = orc.inverse(g.x, kern, v, n0=g.n0, k=g.k, nbr=g.nbr)
+    assert rel(xi2, xi) < 1e-10
+
+
+# ------------------------------------------------------------------ P-3 VJP vs finite differences
+@pytest.mark.parametrize("kind,sigma,ell,jit", KERNELS)
+def test_p3_vjp_matches_central_differences(orc, kind, sigma, ell, jit):
+    n, n0, k = 300, 16, 6
+    x = W.make_points(W.CONFIGS[1], "f64", n)
+    g = orc.build_graph(x, k, n0)
+    xi = W.make_noise(1, n, "f64")
+    vbar = W.make_noise(1, n, "f64", "vbar")
+    jit = max(jit, 1e-8)
+    kern = orc.Kernel(kind, sigma, ell, jit)
+    kw = dict(n0=n0, k=k, nbr=g.nbr, batch_off=g.batch_off)
+    v = orc.forward(g.x, kern, xi, **kw)
+    xibar, tb = orc.vjp(g.x, kern, xi, v, vbar, **kw)
+
+    def f(sig, el, z):
+        return float(vbar @ orc.forward(g.x, orc.Kernel(kind, sig, el, jit), z, **kw))
+
+    h = 1e-6
+    ds = (f(sigma * (1 + h), ell, xi) - f(sigma * (1 - h), ell, xi)) / (2 * h * sigma)
+    dl = (f(sigma, ell * (1 + h), xi) - f(sigma, ell * (1 - h), xi)) / (2 * h * ell)
+    assert abs(tb[0] - ds) / abs(ds) < 1e-7
+    assert abs(tb[1] - dl) / abs(dl) < 1e-6
+    # xi_bar: the map is linear in xi, so one-sided differences are exact up to rounding
+    for j in (0, 5, n0 - 1, n0, n0 + 7, n - 1):
+        e = np.zeros(n)
+        e[j] = 1.0
+        dj = f(sigma, ell, xi + e) - f(sigma, ell, xi)
+        assert abs(xibar[j] - dj) < 1e-9 * max(1.0, abs(dj))
+    # logdet gradient
+    ld, gl = orc.logdet(g.x, kern, n0=n0, k=k, nbr=g.nbr, grad=True)
+    lds = (orc.logdet(g.x, orc.Kernel(kind, sigma * (1 + h), ell, jit), n0=n0, k=k, nbr=g.nbr)
+           - orc.logdet(g.x, orc.Kernel(kind, sigma * (1 - h), ell, jit), n0=n0, k=k, nbr=g.nbr)) / (2 * h * sigma)
+    ldl = (orc.logdet(g.x, orc.Kernel(kind, sigma, ell * (1 + h), jit), n0=n0, k=k, nbr=g.nbr)
+           - orc.logdet(g.x, orc.Kernel(kind, sigma, ell * (1 - h), jit), n0=n0, k=k, nbr=g.nbr)) / (2 * h * ell)
+    assert abs(gl[0] - lds) / abs(lds) < 1e-6
+    assert abs(gl[1] - ldl) / abs(ldl) < 1e-6
+
+
+# ------------------------------------------------------------------ P-4 neighbours by brute force
+@pytest.mark.parametrize("cid,n,k", [(1, 1500, 8), (4, 1200, 32)])
+def test_p4_preceding_knn_against_numpy_brute_force(orc, cid, n, k):
+    cfg = W.CONFIGS[cid]
+    x = W.make_points(cfg, "f32", n).astype(np.float64)
+    x[10] = x[3]            # exact duplicates and equidistant ties must resolve by index
+    x[700] = x[3]
+    perm = orc.order(x)
+    xt = x[perm]
+    n0 = k
+    nbr = orc.knn(xt, k, n0)
+    assert nbr.shape == (n - n0, k)
+    for i in range(n0, n, 7):
+        diff = xt[i][None, :] - xt[:i]
+        sq = diff * diff                                   # numpy elementwise: no FMA, same sum order
+        d2 = sq[:, 0]
+        for j in range(1, xt.shape[1]):
+            d2 = d2 + sq[:, j]
+        want = np.lexsort((np.arange(i), d2))[:k]          # (d2, index) lexicographic
+        got = nbr[i - n0]
+        assert np.all(got < i) and np.all(got >= 0)
+        assert len(set(got.tolist())) == k
+        assert np.array_equal(got, want.astype(np.int32))
+
+
+# ------------------------------------------------------------------ P-5 k = 1 closed form
+@pytest.mark.parametrize("kind,sigma,ell,jit", KERNELS)
+def test_p5_single_neighbour_closed_form(orc, kind, sigma, ell, jit):
+    x = np.array([[0.1, 0.2, 0.3], [0.25, 0.1, 0.35]])
+    r = float(np.linalg.norm(x[0] - x[1]))
+    w, s2 = orc.condition(x, orc.Kernel(kind, sigma, ell, jit), 1, [0])
+    rho = float(np_rho(kind, r, ell))
+    assert abs(w[0] - rho / (1 + jit)) < 1e-14
+    assert abs(s2 - sigma ** 2 * (1 + jit - rho ** 2 / (1 + jit))) < 1e-14 * sigma ** 2
+
+
+def test_rho_and_derivative_values(orc):
+    """kappa closed forms (BASELINE.json) at hand-computable points, and d rho/d ell by differences."""
+    assert abs(orc.rho("se", 0.1, 0.1) - math.exp(-0.5)) < 1e-15
+    assert abs(orc.rho("matern32", 0.05, 0.05) - (1 + math.sqrt(3)) * math.exp(-math.sqrt(3))) < 1e-15
+    assert abs(orc.rho("exp", 0.02, 0.01) - math.exp(-2.0)) < 1e-15
+    for kind in ("se", "matern32", "exp"):
+        assert orc.rho(kind, 0.0, 0.3) == 1.0
+        assert orc.drho_dell(kind, 0.0, 0.3) == 0.0
+        r, ell, h = 0.37, 0.21, 1e-6
+        fd = (orc.rho(kind, r, ell + h) - orc.rho(kind, r, ell - h)) / (2 * h)
+        assert abs(orc.drho_dell(kind, r, ell) - fd) < 1e-8
+
+
+# ------------------------------------------------------------------ P-6 sigma scaling
+def test_p6_sigma_scaling(orc):
+    n, n0, k = 500, 32, 8
+    x = W.make_points(W.CONFIGS[1], "f64", n)
+    g = orc.build_graph(x, k, n0)
+    kw = dict(n0=n0, k=k, nbr=g.nbr, batch_off=g.batch_off)
+    xi = W.make_noise(1, n, "f64")
+    vbar = W.make_noise(1, n, "f64", "vbar")
+    k1 = orc.Kernel("matern32", 1.0, 0.1, 1e-6)
+    k3 = orc.Kernel("matern32", 3.0, 0.1, 1e-6)
+    v1 = orc.forward(g.x, k1, xi, **kw)
+    v3 = orc.forward(g.x, k3, xi, **kw)
+    assert rel(v3, 3.0 * v1) < 1e-13
+    l1 = orc.logdet(g.x, k1, n0=n0, k=k, nbr=g.nbr)
+    l3, g3 = orc.logdet(g.x, k3, n0=n0, k=k, nbr=g.nbr, grad=True)
+    assert abs(l3 - (l1 + 2 * n * math.log(3.0))) < 1e-9
+    assert abs(g3[0] - 2 * n / 3.0) / (2 * n / 3.0) < 1e-10
+    _, tb = orc.vjp(g.x, k3, xi, v3, vbar, **kw)
+    assert abs(tb[0] - float(vbar @ v3) / 3.0) / abs(float(vbar @ v3) / 3.0) < 1e-9
+
+
+# ------------------------------------------------------------------ P-7 power-of-two scale invariance
+def test_p7_power_of_two_scaling_is_bit_exact(orc):
+    n, n0, k = 3000, 64, 8
+    x = W.make_points(W.CONFIGS[3], "f32", n).astype(np.float64)
+    ga = orc.build_graph(x, k, n0)
+    gb = orc.build_graph(2.0 * x, k, n0)
+    assert np.array_equal(ga.perm, gb.perm)
+    assert np.array_equal(ga.nbr, gb.nbr)
+    assert np.array_equal(ga.batch_off, gb.batch_off)
+    xi = W.make_noise(3, n, "f64")
+    for kind in ("se", "matern32", "exp"):
+        va = orc.forward(ga.x, orc.Kernel(kind, 1.0, 0.02, 1e-3), xi, n0=n0, k=k, nbr=ga.nbr)
+        vb = orc.forward(gb.x, orc.Kernel(kind, 1.0, 0.04, 1e-3), xi, n0=n0, k=k, nbr=gb.nbr)
+        assert np.array_equal(va, vb)
+
+
+# ------------------------------------------------------------------ P-8 Markov special case
+def test_p8_markov_exponential_1d(orc):
+    """d=1, exponential kernel, sorted points, c(i)={i-1}: the process is Markov, so Vecchia is exact:
+    v = L xi (dense), logdet = sum_i log(1 - exp(-2 Delta_i / ell))  (sigma = 1, no nugget)."""
+    n, ell = 200, 0.37
+    xs = np.sort(W.uniform(77, 0, 0, n, np.float64))[:, None]
+    xi = W.make_noise(1, n, "f64")
+    kern = orc.Kernel("exp", 1.0, ell, 0.0)
+    rowptr = np.concatenate([[0], np.arange(0, n)]).astype(np.int64)
+    col = np.arange(0, n - 1, dtype=np.int32)
+    v = orc.forward(xs, kern, xi, rowptr=rowptr, col=col)
+    K = np_dense_K(xs, "exp", 1.0, ell, 0.0)
+    v_dense = np.linalg.cholesky(K) @ xi
+    assert rel(v, v_dense) < 1e-11
+    delta = np.diff(xs[:, 0])
+    closed = float(np.sum(np.log1p(-np.exp(-2.0 * delta / ell))))
+    ld = orc.logdet(xs, kern, rowptr=rowptr, col=col)
+    assert abs(ld - closed) / abs(closed) < 1e-12
+
+
+# ------------------------------------------------------------------ P-9 logdet ordering
+def test_p9_logdet_decreases_with_nested_conditioning(orc):
+    """sum log s^2 (Vecchia) >= log det K, non-increasing when conditioning sets are nested."""
+    n = 400
+    x = W.make_points(W.CONFIGS[1], "f64", n)
+    xt = x[orc.order(x)]
+    kern = orc.Kernel("matern32", 1.0, 0.2, 1e-6)
+    _, ld_dense = np.linalg.slogdet(np_dense_K(xt, "matern32", 1.0, 0.2, 1e-6))
+    big = orc.knn(xt, 32, 32)                              # nearest first => prefixes are nested sets
+    prev = None
+    for k in (2, 4, 8, 16, 32):
+        rp = [0]
+        cols = []
+        for i in range(n):
+            c = np.arange(i, dtype=np.int32)[:k] if i < 32 else big[i - 32][:k]
+            if i < 32:                                     # nested for the head too: first min(i,k) points
+                c = np.arange(min(i, k), dtype=np.int32)
+            cols.append(c)
+            rp.append(rp[-1] + c.size)
+        ld = orc.logdet(xt, kern, rowptr=np.array(rp, np.int64), col=np.concatenate(cols).astype(np.int32))
+        assert ld >= ld_dense - 1e-9
+        if prev is not None:
+            assert ld <= prev + 1e-9
+        prev = ld
+
+
+# ------------------------------------------------------------------ P-11 order
+def _golden_orders():
+    out = []
+    with open(os.path.join(HERE, "golden", "order_examples.txt")) as f:
+        for line in f:
+            if line.startswith("#") or ":" not in line:
+                continue
+            n, seq = line.split(":")
+            out.append((int(n), [int(t) for t in seq.split()]))
+    return out
+
+
+def test_p11_order_worked_examples(orc):
+    for n, seq in _golden_orders():
+        x = np.arange(1, n + 1, dtype=np.float64)[:, None]
+        perm = orc.order(x)
+        assert (perm + 1).tolist() == seq
+
+
+def _bitrev(q, bits):
+    r = 0
+    for _ in range(bits):
+        r = (r << 1) | (q & 1)
+        q >>= 1
+    return r
+
+
+@pytest.mark.parametrize("m,d", [(7, 3), (9, 2)])
+def test_p11_full_tree_is_bit_reversed_heap_order(orc, m, d):
+    """with all levels full the order is the per-level bit reversal of the textbook
+    median-split balanced k-d tree in heap order."""
+    n = 2 ** m - 1
+    x = W.make_points(W.CONFIGS[1] if d == 3 else W.CONFIGS[4], "f64", n)
+
+    heap = np.empty(n, dtype=np.int64)
+
+    def build(node, ids, level):                           # textbook recursive median split
+        if ids.size == 0:
+            return
+        dim = level % d
+        ids = ids[np.lexsort((ids, x[ids, dim]))]
+        mid = ids.size // 2                                # perfect tree: sizes are 2^j - 1
+        heap[node] = ids[mid]
+        build(2 * node + 1, ids[:mid], level + 1)
+        build(2 * node + 2, ids[mid + 1:], level + 1)
+
+    build(0, np.arange(n), 0)
+    want = np.empty(n, dtype=np.int64)
+    for l in range(m):
+        for q in range(2 ** l):
+            want[2 ** l - 1 + _bitrev(q, l)] = heap[2 ** l - 1 + q]
+    assert np.array_equal(orc.order(x), want)
+
+
+@pytest.mark.parametrize("n,d", [(1, 3), (2, 3), (3, 2), (100, 3), (1000, 2), (4097, 3)])
+def test_p11_kd_invariants_and_prefix_validity(orc, n, d):
+    x = W.make_points(W.CONFIGS[3] if d == 3 else W.CONFIGS[4], "f32", n).astype(np.float64)
+    if n > 50:
+        x[5] = x[17]                                       # duplicate coordinates: ties by user id
+    perm = orc.order(x)
+    assert sorted(perm.tolist()) == list(range(n))
+    sz = orc.subtree_sizes(n)
+    members = [None] * n
+    for i in range(n - 1, -1, -1):                          # child index > parent index (prefix validity)
+        l = int(math.floor(math.log2(i + 1)))
+        kids = [c for c in (i + 2 ** l, i + 2 ** (l + 1)) if c < n]
+        assert all(c > i for c in kids)
+        mem = [[perm[i]]] + [members[c] for c in kids]
+        members[i] = [u for part in mem for u in part]
+        assert len(members[i]) == sz[i]
+        dim = l % d
+        key = lambda u: (x[u, dim], u)
+        left, right = i + 2 ** l, i + 2 ** (l + 1)
+        if left < n:
+            assert max(key(u) for u in members[left]) < key(perm[i])
+        if right < n:
+            assert min(key(u) for u in members[right]) > key(perm[i])
+        for c in kids:
+            members[c] = members[c] if n < 200 else members[c]
+    # closed form of the subtree sizes used by the GPU builder
+    lam = int(math.floor(math.log2(n)))
+    mlast = n - (2 ** lam - 1)
+    for i in range(n):
+        l = int(math.floor(math.log2(i + 1)))
+        p = i - (2 ** l - 1)
+        s = 1 if l == lam else (2 ** (lam - l) - 1) + max(0, -((p - mlast) // 2 ** l))
+        assert s == sz[i]
+
+
+# ------------------------------------------------------------------ P-12 depth
+def test_p12_depth_sequential_equals_fixed_point_and_batches(orc):
+    n, n0, k = 6000, 64, 8
+    x = W.make_points(W.CONFIGS[3], "f32", n).astype(np.float64)
+    perm = orc.order(x)
+    xt = x[perm]
+    nbr = orc.knn(xt, k, n0)
+    dep = orc.depth(nbr, n, n0)
+    dep2, sweeps = orc.depth_fixed_point(nbr, n, n0)
+    assert np.array_equal(dep, dep2)
+    assert sweeps <= dep.max() + 1
+    g = orc.depth_sort(xt, nbr, dep, perm, n0)
+    # P-10 invariants
+    assert g.batch_off[0] == n0 and g.batch_off[-1] == n and np.all(np.diff(g.batch_off) > 0)
+    pos = np.arange(n0, n)
+    assert np.all(g.nbr < pos[:, None])
+    for b in range(len(g.batch_off) - 1):
+        lo, hi = g.batch_off[b], g.batch_off[b + 1]
+        assert np.all(g.depth[lo:hi] == b + 1)
+        assert np.all(g.nbr[lo - n0:hi - n0] < lo)                         # only earlier batches
+        assert np.all((g.depth[g.nbr[lo - n0:hi - n0]] == b).any(axis=1))  # some neighbour in batch b-1
+    # generating in depth-sorted order "does not change any conditioning relationships"
+    kern = orc.Kernel("matern32", 1.0, 0.05, 1e-4)
+    xi_user = W.make_noise(3, n, "f64")
+    v_tree = orc.forward(xt, kern, xi_user[perm], n0=n0, k=k, nbr=nbr)
+    v_graph = orc.forward(g.x, kern, xi_user[g.perm], n0=n0, k=k, nbr=g.nbr, batch_off=g.batch_off)
+    vu_a = np.empty(n)
+    vu_a[perm] = v_tree
+    vu_b = np.empty(n)
+    vu_b[g.perm] = v_graph
+    assert rel(vu_a, vu_b) < 1e-12
+
+
+# ------------------------------------------------------------------ P-13 (qualitative)
+def test_p13_graphgp_order_gives_fewer_batches_than_random_order(orc):
+    n, k, n0 = 10000, 16, 50
+    x = W.make_gaussian_blob(n, 3, "f64")
+    g = orc.build_graph(x, k, n0)
+    L_graphgp = len(g.batch_off) - 1
+    rng_perm = np.argsort(W.raw_u64(5, 0, 0, n), kind="stable")
+    nbr = orc.knn(x[rng_perm], k, n0)
+    L_random = int(orc.depth(nbr, n, n0).max())
+    lam = int(math.floor(math.log2(n)))
+    slots = 2 ** (lam + 1) - 1                               # standard (heap) order of the same tree
+    heap = np.empty(slots, dtype=np.int64)
+    for i in range(slots):
+        l = int(math.floor(math.log2(i + 1)))
+        q = i - (2 ** l - 1)
+        heap[i] = 2 ** l - 1 + _bitrev(q, l)                 # heap slot q at level l <- bit-reversed position
+    perm = orc.order(x)
+    valid = heap < n                                         # last level: only positions < m exist
+    std_order = perm[heap[valid]]
+    assert sorted(std_order.tolist()) == list(range(n))
+    nbr_std = orc.knn(x[std_order], k, n0)
+    L_std = int(orc.depth(nbr_std, n, n0).max())
+    assert L_graphgp < L_random < L_std
+
+
+# ------------------------------------------------------------------ P-14 long double
+@pytest.mark.parametrize("cid", [1, 2, 3])
+def test_p14_double_agrees_with_long_double(orc, cid):
+    cfg = W.CONFIGS[cid]
+    n = 4096
+    x = W.make_points(cfg, "f32" if cid != 1 else "f64", n).astype(np.float64)
+    g = orc.build_graph(x, cfg.k, 64)
+    kern = orc.Kernel(cfg.kind, cfg.sigma, cfg.ell, cfg.jitter)
+    xi = W.make_noise(cid, n, "f64")
+    kw = dict(n0=g.n0, k=g.k, nbr=g.nbr)
+    v = orc.forward(g.x, kern, xi, **kw)
+    v_ld = orc.forward(g.x, kern, xi, long_double=True, **kw)
+    assert rel(v, v_ld) < 1e-10
+    ld, ld_ld = orc.logdet(g.x, kern, **kw), orc.logdet(g.x, kern, long_double=True, **kw)
+    assert abs(ld - ld_ld) / abs(ld_ld) < 1e-12
