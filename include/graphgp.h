@@ -1,0 +1,149 @@
+/* graphgp.h — C ABI of the B200-native GraphGP hot path (Vecchia conditioning).
+ *
+ * Source of every operation: arxiv/paper_2606_11402 as extracted in PAPER.md
+ *   Eq. 1, Eq. 2, Alg. 1,
+ *   §2.2 ordering/batches, §2.3 implementation.
+ * Scope table: SURVEY.md §8(b).  Readings of silent/garbled passages: DESIGN.md §3.
+ *
+ * Conventions
+ *   - 0-based indices.  All per-point arrays (x, xi, v, v_bar, xi_bar) are in GRAPH order: the
+ *     paper's bit-reversed k-d tree order stably sorted by depth, head first.
+ *   - K_ab = sigma^2 [ rho(|x_a - x_b|) + jitter * delta_ab ]  (relative nugget, R-7).
+ *   - "device" = CUDA device memory of the current device; "host" = ordinary host memory.
+ *   - Ownership: the caller owns every buffer, including the workspace.  The library allocates
+ *     nothing on these calls and keeps no global state.  Calls are asynchronous on `cuda_stream`
+ *     (a cudaStream_t passed as void*; NULL = default stream) unless stated otherwise.
+ *   - Errors: return codes only.  Argument errors are synchronous.  A numerical failure (a pivot or
+ *     conditional variance that is not positive and finite) writes NaN for that point and increments
+ *     a device counter that gp_check_errors() reads.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point returns GP_ERR_CUDA.
+ */
+#ifndef GRAPHGP_H_
+#define GRAPHGP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  GP_OK = 0,
+  GP_ERR_INVALID_ARG = 1,
+  GP_ERR_UNSUPPORTED = 2, /* (k, d, dtype) outside what the library handles (k <= 64, d <= 4) */
+  GP_ERR_NOT_PD = 3,
+  GP_ERR_CUDA = 4,
+  GP_ERR_WORKSPACE = 5 /* ws == NULL or ws_bytes < gp_workspace_bytes() */
+} gp_status;
+
+typedef enum { GP_KERNEL_SE = 0, GP_KERNEL_MATERN32 = 1, GP_KERNEL_EXP = 2 } gp_kernel_kind;
+typedef enum { GP_F32 = 0, GP_F64 = 1 } gp_dtype;
+typedef enum { GP_OP_FORWARD = 0, GP_OP_INVERSE = 1, GP_OP_LOGDET = 2, GP_OP_VJP = 3, GP_OP_BUILD = 4 } gp_op;
+
+/* gp_graph.flags */
+enum {
+  GP_FLAG_PER_BATCH_LAUNCH = 1, /* forward/VJP: one launch per batch (Alg. 1 lines 2-8 literally) instead of
+                                   the single dataflow launch; results agree to rounding */
+  GP_FLAG_GENERIC_KERNEL = 2    /* force the runtime-(k,d,kind) kernel even where a specialised one exists */
+};
+
+/* Stationary covariance kappa(r) = sigma^2 rho(r); rho:
+ *   SE        exp(-r^2 / (2 ell^2))
+ *   MATERN32  (1 + sqrt(3) r / ell) exp(-sqrt(3) r / ell)
+ *   EXP       exp(-r / ell)                                   (BASELINE.json configs) */
+typedef struct {
+  int32_t kind; /* gp_kernel_kind */
+  double sigma, ell, jitter;
+} gp_kernel;
+
+/* The inputs of Alg. 1 `Require` except the noise. */
+typedef struct {
+  int64_t n;         /* number of points N                                                            */
+  int64_t n0;        /* size of the dense initial block (Alg. 1 line 1); k <= n0 <= n    */
+  int32_t d;         /* spatial dimension, 1..4                                                        */
+  int32_t k;         /* neighbours per point, 1..64                                                    */
+  int32_t n_batches; /* L                                                                              */
+  int32_t dtype;     /* gp_dtype of x, xi, v, v_bar, xi_bar                                            */
+  int32_t flags;     /* GP_FLAG_*                                                                      */
+  int32_t reserved;
+  const void* x;            /* device, [n][d] row-major, graph order, dtype                           */
+  const int32_t* nbr;       /* device, [n - n0][k] row-major; row r belongs to point i = n0 + r; every
+                               entry is a graph position < batch start of i; order inside a row is free */
+  const int64_t* batch_off; /* HOST, [n_batches + 1]; batch_off[0] = n0, strictly increasing,
+                               batch_off[n_batches] = n.  Points of one batch are conditionally
+                               independent.                                              */
+} gp_graph;
+
+/* Bytes of workspace `op` needs for this graph (0 on invalid arguments). */
+size_t gp_workspace_bytes(const gp_graph* g, int32_t op);
+
+/* Forward generation, Alg. 1:  v[0:n0] = chol(K_head) xi[0:n0];  for each batch, for
+ * every point i in it:  v_i = K_ic K_cc^-1 v_c + sqrt(K_ii - K_ic K_cc^-1 K_ci) xi_i   (Eq. 2).
+ * xi: device [n] (in);  v: device [n] (out).                                                          */
+gp_status gp_forward(const gp_graph* g, const gp_kernel* kern, const void* xi, void* v, void* ws,
+                     size_t ws_bytes, void* cuda_stream);
+
+/* Inverse ("easily parallelized"):  xi_i = (v_i - K_ic K_cc^-1 v_c) / s_i for all
+ * i at once; head: xi[0:n0] = chol(K_head)^-1 v[0:n0].   v: device [n] (in);  xi: device [n] (out).   */
+gp_status gp_inverse(const gp_graph* g, const gp_kernel* kern, const void* v, void* xi, void* ws,
+                     size_t ws_bytes, void* cuda_stream);
+
+/* Log-determinant of the Vecchia covariance:  sum_i log s_i^2  (+ log det K_head).
+ * logdet_dev: device double[1] (out).  dlogdet_dtheta_dev: device double[2] = d/dsigma, d/dell, or NULL. */
+gp_status gp_logdet(const gp_graph* g, const gp_kernel* kern, double* logdet_dev, double* dlogdet_dtheta_dev,
+                    void* ws, size_t ws_bytes, void* cuda_stream);
+
+/* Vector-Jacobian product of gp_forward ("backward derivatives"): given xi, v = forward(xi)
+ * and a cotangent v_bar, returns xi_bar [n] and theta_bar = (d/dsigma, d/dell) of <v_bar, forward(xi; theta)>.
+ * xi, v, v_bar: device [n] (in);  xi_bar: device [n] (out);  theta_bar_dev: device double[2] (out).
+ * Floating-point atomics make the last bits of xi_bar/theta_bar run-dependent.                        */
+gp_status gp_vjp(const gp_graph* g, const gp_kernel* kern, const void* xi, const void* v, const void* v_bar,
+                 void* xi_bar, double* theta_bar_dev, void* ws, size_t ws_bytes, void* cuda_stream);
+
+/* End-to-end variants with HOST input/output vectors: copy the [n] input host->device into `in_dev`,
+ * run the op, copy the [n] result device->host, all on `cuda_stream` (pinned host memory makes the
+ * copies asynchronous).  The graph stays device-resident.  in_dev/out_dev: device staging, [n] each.  */
+gp_status gp_forward_host(const gp_graph* g, const gp_kernel* kern, const void* xi_host, void* v_host,
+                          void* in_dev, void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream);
+gp_status gp_inverse_host(const gp_graph* g, const gp_kernel* kern, const void* v_host, void* xi_host,
+                          void* in_dev, void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream);
+
+/* Graph construction, separately timed, "plain":
+ *   order   bit-reversed left-balanced k-d tree: node i at level l has children i+2^l, i+2^(l+1);
+ *           split dimension = level mod d; ties by (coordinate, user id)             (R-3, R-4)
+ *   kNN     k nearest among PRECEDING points in that order, ranked by (fp64 FMA-free squared distance,
+ *           tree index)                                                                   (R-5)
+ *   depth   d_i = 1 + max_{j in c(i)} d_j by parallel fixed point; head depth 0
+ *   sort    graph order = tree order stably sorted by depth; with GP_BUILD_SPATIAL_BATCHES points inside
+ *           a batch are additionally ordered by k-d in-order rank (any order inside a batch is legal,
+ *           PAPER.md:43) so that neighbouring threads gather neighbouring memory.
+ * x_user: device [n][d] dtype (in).  Outputs (device unless noted): perm [n] graph position -> user id;
+ * x_graph [n][d] dtype; nbr [n-n0][k]; depth [n] (graph order); batch_off_host: HOST int64
+ * [max_batches+1]; n_batches: HOST.  Synchronises the stream before returning (batch_off is host data).
+ * Requires n < 2^31.                                                                                   */
+enum { GP_BUILD_SPATIAL_BATCHES = 1 };
+gp_status gp_graph_build(const void* x_user, int64_t n, int32_t d, int32_t k, int64_t n0, int32_t dtype,
+                         int32_t build_flags, int64_t* perm, void* x_graph, int32_t* nbr, int32_t* depth,
+                         int64_t* batch_off_host, int32_t max_batches, int32_t* n_batches, void* ws,
+                         size_t ws_bytes, void* cuda_stream);
+size_t gp_graph_build_workspace_bytes(int64_t n, int32_t d, int32_t k, int32_t dtype);
+/* Optional per-stage device times of the last gp_graph_build on this workspace, milliseconds:
+ * [0] order, [1] kNN, [2] depth, [3] depth sort + remap.  HOST double[4].                              */
+gp_status gp_graph_build_times(void* ws, double* ms4_host);
+
+/* Number of points whose conditional was not positive definite in the last op that used `ws`.
+ * Synchronous: copies one counter from the device (the caller must have synchronised the stream).     */
+gp_status gp_check_errors(void* ws, int64_t* n_bad_points);
+
+const char* gp_status_string(gp_status s);
+
+/* Diagnostics: 1 if (dtype, k, d, kind) has a register-resident specialised kernel, else 0.           */
+int32_t gp_has_specialised(int32_t dtype, int32_t k, int32_t d, int32_t kind);
+/* Number of kernels launched by the library in this process so far (for bench.py's gpu_launches).    */
+int64_t gp_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRAPHGP_H_ */

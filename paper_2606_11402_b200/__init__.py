@@ -1,0 +1,287 @@
+"""paper_2606_11402_b200 — thin Python binding over libgraphgp.so (include/graphgp.h).
+
+Argument marshalling only: every step of the Vecchia conditioning path runs in the CUDA kernels of
+csrc/.  PyTorch supplies device memory and streams.  There is no CPU fallback: if the extension is
+missing or there is no CUDA device the calls raise.
+
+Names follow the C ABI: gp_forward, gp_inverse, gp_logdet, gp_vjp, gp_graph_build.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass, field
+
+import numpy as np
+
+from .build import LIB, build_library
+
+GP_OK, GP_ERR_INVALID_ARG, GP_ERR_UNSUPPORTED, GP_ERR_NOT_PD, GP_ERR_CUDA, GP_ERR_WORKSPACE = range(6)
+GP_F32, GP_F64 = 0, 1
+GP_OP_FORWARD, GP_OP_INVERSE, GP_OP_LOGDET, GP_OP_VJP, GP_OP_BUILD = range(5)
+GP_FLAG_PER_BATCH_LAUNCH, GP_FLAG_GENERIC_KERNEL = 1, 2
+GP_BUILD_SPATIAL_BATCHES = 1
+KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
+
+EXPORTS = ["gp_workspace_bytes", "gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host",
+           "gp_inverse_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
+           "gp_check_errors", "gp_status_string", "gp_has_specialised", "gp_launch_count"]
+
+
+class GraphGPError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        super().__init__(f"{where}: {status_string(status)} (gp_status {status})")
+
+
+class _Kernel(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("sigma", C.c_double), ("ell", C.c_double), ("jitter", C.c_double)]
+
+
+class _Graph(C.Structure):
+    _fields_ = [("n", C.c_int64), ("n0", C.c_int64), ("d", C.c_int32), ("k", C.c_int32),
+                ("n_batches", C.c_int32), ("dtype", C.c_int32), ("flags", C.c_int32), ("reserved", C.c_int32),
+                ("x", C.c_void_p), ("nbr", C.c_void_p), ("batch_off", C.c_void_p)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libgraphgp.so (fails loudly if it has not been built: run `python -m paper_2606_11402_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB):
+            raise ImportError(f"{LIB} is missing: build it with `python -m paper_2606_11402_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB)
+        L.gp_workspace_bytes.restype = C.c_size_t
+        L.gp_workspace_bytes.argtypes = [C.POINTER(_Graph), C.c_int32]
+        L.gp_graph_build_workspace_bytes.restype = C.c_size_t
+        L.gp_graph_build_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.c_int32, C.c_int32]
+        L.gp_status_string.restype = C.c_char_p
+        L.gp_status_string.argtypes = [C.c_int]
+        L.gp_launch_count.restype = C.c_int64
+        L.gp_has_specialised.restype = C.c_int32
+        L.gp_has_specialised.argtypes = [C.c_int32] * 4
+        vp, sz = C.c_void_p, C.c_size_t
+        gk = [C.POINTER(_Graph), C.POINTER(_Kernel)]
+        L.gp_forward.argtypes = gk + [vp, vp, vp, sz, vp]
+        L.gp_inverse.argtypes = gk + [vp, vp, vp, sz, vp]
+        L.gp_logdet.argtypes = gk + [vp, vp, vp, sz, vp]
+        L.gp_vjp.argtypes = gk + [vp, vp, vp, vp, vp, vp, sz, vp]
+        L.gp_forward_host.argtypes = gk + [vp, vp, vp, vp, vp, sz, vp]
+        L.gp_inverse_host.argtypes = gk + [vp, vp, vp, vp, vp, sz, vp]
+        L.gp_graph_build.argtypes = [vp, C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32, C.c_int32, vp, vp,
+                                     vp, vp, vp, C.c_int32, C.POINTER(C.c_int32), vp, sz, vp]
+        L.gp_graph_build_times.argtypes = [vp, vp]
+        L.gp_check_errors.argtypes = [vp, C.POINTER(C.c_int64)]
+        for name in ("gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host", "gp_inverse_host",
+                     "gp_graph_build", "gp_graph_build_times", "gp_check_errors"):
+            getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def status_string(status: int) -> str:
+    return lib().gp_status_string(int(status)).decode()
+
+
+def launch_count() -> int:
+    return int(lib().gp_launch_count())
+
+
+def has_specialised(dtype: str, k: int, d: int, kind: str) -> bool:
+    return bool(lib().gp_has_specialised(GP_F64 if dtype == "f64" else GP_F32, k, d, KIND_ID[kind]))
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2606_11402_b200 needs a CUDA device (no CPU fallback)")
+    return torch
+
+
+@dataclass
+class Kernel:
+    kind: str
+    sigma: float
+    ell: float
+    jitter: float
+
+    def c(self) -> _Kernel:
+        return _Kernel(KIND_ID[self.kind], float(self.sigma), float(self.ell), float(self.jitter))
+
+
+@dataclass
+class Graph:
+    """Device-resident generation graph in GRAPH order (Alg. 1 `Require`)."""
+    x: "object"              # torch [n, d] float32/float64, cuda
+    nbr: "object"            # torch [n - n0, k] int32, cuda
+    batch_off: np.ndarray    # host int64 [L + 1]
+    n0: int
+    flags: int = 0
+    perm: "object" = None    # torch [n] int64 graph position -> user id (builder output)
+    depth: "object" = None
+    _ws: dict = field(default_factory=dict, repr=False)
+
+    @property
+    def n(self) -> int:
+        return int(self.x.shape[0])
+
+    @property
+    def d(self) -> int:
+        return int(self.x.shape[1])
+
+    @property
+    def k(self) -> int:
+        return int(self.nbr.shape[1])
+
+    @property
+    def dtype_id(self) -> int:
+        torch = _torch()
+        return GP_F64 if self.x.dtype == torch.float64 else GP_F32
+
+    def c(self) -> _Graph:
+        self.batch_off = np.ascontiguousarray(self.batch_off, dtype=np.int64)
+        nb = max(self.batch_off.size - 1, 0)
+        return _Graph(self.n, int(self.n0), self.d, self.k, nb, self.dtype_id, int(self.flags), 0,
+                      self.x.data_ptr(), self.nbr.data_ptr() if self.nbr.numel() else None,
+                      self.batch_off.ctypes.data if self.batch_off.size else None)
+
+    def workspace(self, op: int):
+        """A cached, caller-side workspace tensor for `op` (the library itself never allocates)."""
+        torch = _torch()
+        g = self.c()
+        need = int(lib().gp_workspace_bytes(C.byref(g), op))
+        if need == 0:
+            raise GraphGPError(GP_ERR_INVALID_ARG, "gp_workspace_bytes")
+        ws = self._ws.get(op)
+        if ws is None or ws.numel() < need:
+            ws = torch.empty(need, dtype=torch.uint8, device=self.x.device)
+            self._ws[op] = ws
+        return ws
+
+
+def graph_from_arrays(x, nbr, batch_off, n0, dtype="f32", device="cuda", flags=0) -> Graph:
+    """Upload host arrays (e.g. a graph made elsewhere) as a device-resident Graph."""
+    torch = _torch()
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    xt = torch.as_tensor(np.ascontiguousarray(x), device=device).to(tdt).contiguous()
+    k = nbr.shape[1]
+    nt = torch.as_tensor(np.ascontiguousarray(nbr, dtype=np.int32), device=device).contiguous().reshape(-1, k)
+    return Graph(x=xt, nbr=nt, batch_off=np.ascontiguousarray(batch_off, dtype=np.int64), n0=int(n0), flags=flags)
+
+
+def _stream_ptr(stream):
+    torch = _torch()
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def _check(status: int, where: str):
+    if status != GP_OK:
+        raise GraphGPError(status, where)
+
+
+def check_errors(ws) -> int:
+    """Synchronise, then return the number of points whose conditional was not positive definite."""
+    torch = _torch()
+    torch.cuda.synchronize()
+    nbad = C.c_int64(0)
+    st = lib().gp_check_errors(C.c_void_p(ws.data_ptr()), C.byref(nbad))
+    if st not in (GP_OK, GP_ERR_NOT_PD):
+        raise GraphGPError(st, "gp_check_errors")
+    return int(nbad.value)
+
+
+def gp_forward(graph: Graph, kern: Kernel, xi, out=None, stream=None):
+    """v = forward(xi): Alg. 1.  xi, v: device [n] in graph order."""
+    torch = _torch()
+    v = torch.empty_like(xi) if out is None else out
+    ws = graph.workspace(GP_OP_FORWARD)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_forward(C.byref(g), C.byref(k), xi.data_ptr(), v.data_ptr(), ws.data_ptr(), ws.numel(),
+                            _stream_ptr(stream)), "gp_forward")
+    return v
+
+
+def gp_inverse(graph: Graph, kern: Kernel, v, out=None, stream=None):
+    """xi = inverse(v)."""
+    torch = _torch()
+    xi = torch.empty_like(v) if out is None else out
+    ws = graph.workspace(GP_OP_INVERSE)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_inverse(C.byref(g), C.byref(k), v.data_ptr(), xi.data_ptr(), ws.data_ptr(), ws.numel(),
+                            _stream_ptr(stream)), "gp_inverse")
+    return xi
+
+
+def gp_logdet(graph: Graph, kern: Kernel, grad: bool = False, stream=None):
+    """log det of the Vecchia covariance (device double[1]); with grad=True also d/d(sigma, ell) (double[2])."""
+    torch = _torch()
+    out = torch.empty(1, dtype=torch.float64, device=graph.x.device)
+    gout = torch.empty(2, dtype=torch.float64, device=graph.x.device) if grad else None
+    ws = graph.workspace(GP_OP_VJP if grad else GP_OP_LOGDET)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_logdet(C.byref(g), C.byref(k), out.data_ptr(), gout.data_ptr() if grad else None,
+                           ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "gp_logdet")
+    return (out, gout) if grad else out
+
+
+def gp_vjp(graph: Graph, kern: Kernel, xi, v, v_bar, stream=None):
+    """VJP of gp_forward: returns (xi_bar [n], theta_bar double[2] = d/dsigma, d/dell)."""
+    torch = _torch()
+    xi_bar = torch.empty_like(xi)
+    tb = torch.empty(2, dtype=torch.float64, device=graph.x.device)
+    ws = graph.workspace(GP_OP_VJP)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_vjp(C.byref(g), C.byref(k), xi.data_ptr(), v.data_ptr(), v_bar.data_ptr(), xi_bar.data_ptr(),
+                        tb.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "gp_vjp")
+    return xi_bar, tb
+
+
+def gp_forward_host(graph: Graph, kern: Kernel, xi_host, v_host, in_dev, out_dev, stream=None):
+    """End-to-end forward with HOST (pinned) xi / v: H2D copy, forward, D2H copy on one stream."""
+    ws = graph.workspace(GP_OP_FORWARD)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_forward_host(C.byref(g), C.byref(k), xi_host.data_ptr(), v_host.data_ptr(), in_dev.data_ptr(),
+                                 out_dev.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
+           "gp_forward_host")
+    return v_host
+
+
+def gp_inverse_host(graph: Graph, kern: Kernel, v_host, xi_host, in_dev, out_dev, stream=None):
+    ws = graph.workspace(GP_OP_INVERSE)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_inverse_host(C.byref(g), C.byref(k), v_host.data_ptr(), xi_host.data_ptr(), in_dev.data_ptr(),
+                                 out_dev.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
+           "gp_inverse_host")
+    return xi_host
+
+
+def gp_graph_build(x_user, k: int, n0: int, build_flags: int = GP_BUILD_SPATIAL_BATCHES, max_batches: int = 1 << 16,
+                   stream=None) -> Graph:
+    """Build order, preceding-kNN graph, depths and batches on the GPU.  x_user: device [n, d]."""
+    torch = _torch()
+    x_user = x_user.contiguous()
+    n, d = int(x_user.shape[0]), int(x_user.shape[1])
+    dt = GP_F64 if x_user.dtype == torch.float64 else GP_F32
+    dev = x_user.device
+    perm = torch.empty(n, dtype=torch.int64, device=dev)
+    xg = torch.empty_like(x_user)
+    nbr = torch.empty((max(n - n0, 0), k), dtype=torch.int32, device=dev)
+    depth = torch.empty(n, dtype=torch.int32, device=dev)
+    boff = np.zeros(max_batches + 1, dtype=np.int64)
+    nb = C.c_int32(0)
+    need = int(lib().gp_graph_build_workspace_bytes(n, d, k, dt))
+    ws = torch.empty(max(need, 256), dtype=torch.uint8, device=dev)
+    _check(lib().gp_graph_build(x_user.data_ptr(), n, d, k, n0, dt, build_flags, perm.data_ptr(), xg.data_ptr(),
+                                nbr.data_ptr() if nbr.numel() else None, depth.data_ptr(), boff.ctypes.data,
+                                max_batches, C.byref(nb), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
+           "gp_graph_build")
+    times = np.zeros(4, dtype=np.float64)
+    lib().gp_graph_build_times(ws.data_ptr(), times.ctypes.data)
+    g = Graph(x=xg, nbr=nbr, batch_off=boff[: nb.value + 1].copy(), n0=int(n0), perm=perm, depth=depth)
+    g.build_ms = times
+    return g

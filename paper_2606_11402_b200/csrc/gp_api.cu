@@ -1,0 +1,138 @@
+// C ABI of include/graphgp.h: argument validation, workspace carving, dispatch.  No torch types,
+// no allocation, no global state except the launch counter used by bench.py's gpu_launches.
+#include <atomic>
+#include <cstring>
+
+#include "gp_common.cuh"
+
+namespace gp {
+static std::atomic<long long> g_launches{0};
+void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+static gp_status validate(const gp_graph* g, const gp_kernel* kern) {
+  if (!g || !kern) return GP_ERR_INVALID_ARG;
+  if (g->n <= 0 || g->n0 < 0 || g->n0 > g->n) return GP_ERR_INVALID_ARG;
+  if (g->dtype != GP_F32 && g->dtype != GP_F64) return GP_ERR_INVALID_ARG;
+  if (g->d < 1 || g->k < 1) return GP_ERR_INVALID_ARG;
+  if (g->d > kMaxD || g->k > kMaxK) return GP_ERR_UNSUPPORTED;
+  if (g->n >= (1LL << 31)) return GP_ERR_UNSUPPORTED;
+  if (g->n0 < g->k && g->n0 < g->n) return GP_ERR_INVALID_ARG;  // every row needs k predecessors
+  if (g->n_batches < 0 || g->n_batches > kMaxBatches) return GP_ERR_INVALID_ARG;
+  if (!g->x) return GP_ERR_INVALID_ARG;
+  if (g->n > g->n0) {
+    if (!g->nbr || !g->batch_off || g->n_batches < 1) return GP_ERR_INVALID_ARG;
+    if (g->batch_off[0] != g->n0 || g->batch_off[g->n_batches] != g->n) return GP_ERR_INVALID_ARG;
+    for (int b = 0; b < g->n_batches; ++b)
+      if (g->batch_off[b + 1] <= g->batch_off[b]) return GP_ERR_INVALID_ARG;
+  } else if (g->n_batches != 0 && !g->batch_off) {
+    return GP_ERR_INVALID_ARG;
+  }
+  if (kern->kind < 0 || kern->kind > 2) return GP_ERR_INVALID_ARG;
+  if (!(kern->sigma > 0.0) || !(kern->ell > 0.0) || !(kern->jitter >= 0.0)) return GP_ERR_INVALID_ARG;
+  return GP_OK;
+}
+
+static gp_status make_ctx(const gp_graph* g, const gp_kernel* kern, int op, void* ws, size_t ws_bytes,
+                          void* stream, OpCtx* out) {
+  GP_OK_OR_RETURN(validate(g, kern));
+  WsLayout lay = ws_layout(g, op);
+  if (!ws || ws_bytes < lay.total || (((uintptr_t)ws) & 255) != 0) return GP_ERR_WORKSPACE;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return GP_ERR_CUDA;
+  out->g = g; out->kern = kern; out->ws = (char*)ws; out->lay = lay; out->st = (cudaStream_t)stream;
+  return GP_OK;
+}
+}  // namespace gp
+
+using namespace gp;
+
+extern "C" {
+
+size_t gp_workspace_bytes(const gp_graph* g, int32_t op) {
+  if (!g || g->n <= 0 || g->n0 < 0 || g->n0 > g->n || g->n_batches < 0 || op < GP_OP_FORWARD || op > GP_OP_VJP)
+    return 0;
+  return ws_layout(g, op).total;
+}
+
+gp_status gp_forward(const gp_graph* g, const gp_kernel* kern, const void* xi, void* v, void* ws, size_t ws_bytes,
+                     void* cuda_stream) {
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_FORWARD, ws, ws_bytes, cuda_stream, &c));
+  if (!xi || !v) return GP_ERR_INVALID_ARG;
+  return run_forward(c, xi, v);
+}
+
+gp_status gp_inverse(const gp_graph* g, const gp_kernel* kern, const void* v, void* xi, void* ws, size_t ws_bytes,
+                     void* cuda_stream) {
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_INVERSE, ws, ws_bytes, cuda_stream, &c));
+  if (!xi || !v) return GP_ERR_INVALID_ARG;
+  return run_inverse(c, v, xi);
+}
+
+gp_status gp_logdet(const gp_graph* g, const gp_kernel* kern, double* logdet_dev, double* dlogdet_dtheta_dev,
+                    void* ws, size_t ws_bytes, void* cuda_stream) {
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, dlogdet_dtheta_dev ? GP_OP_VJP : GP_OP_LOGDET, ws, ws_bytes, cuda_stream, &c));
+  if (!logdet_dev) return GP_ERR_INVALID_ARG;
+  return run_logdet(c, logdet_dev, dlogdet_dtheta_dev);
+}
+
+gp_status gp_vjp(const gp_graph* g, const gp_kernel* kern, const void* xi, const void* v, const void* v_bar,
+                 void* xi_bar, double* theta_bar_dev, void* ws, size_t ws_bytes, void* cuda_stream) {
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_VJP, ws, ws_bytes, cuda_stream, &c));
+  if (!xi || !v || !v_bar || !xi_bar || !theta_bar_dev) return GP_ERR_INVALID_ARG;
+  return run_vjp(c, xi, v, v_bar, xi_bar, theta_bar_dev);
+}
+
+gp_status gp_forward_host(const gp_graph* g, const gp_kernel* kern, const void* xi_host, void* v_host, void* in_dev,
+                          void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream) {
+  if (!g || !xi_host || !v_host || !in_dev || !out_dev) return GP_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  size_t bytes = (size_t)g->n * dtype_bytes(g->dtype);
+  GP_CUDA_OK(cudaMemcpyAsync(in_dev, xi_host, bytes, cudaMemcpyHostToDevice, st));
+  GP_OK_OR_RETURN(gp_forward(g, kern, in_dev, out_dev, ws, ws_bytes, cuda_stream));
+  GP_CUDA_OK(cudaMemcpyAsync(v_host, out_dev, bytes, cudaMemcpyDeviceToHost, st));
+  return GP_OK;
+}
+
+gp_status gp_inverse_host(const gp_graph* g, const gp_kernel* kern, const void* v_host, void* xi_host, void* in_dev,
+                          void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream) {
+  if (!g || !xi_host || !v_host || !in_dev || !out_dev) return GP_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  size_t bytes = (size_t)g->n * dtype_bytes(g->dtype);
+  GP_CUDA_OK(cudaMemcpyAsync(in_dev, v_host, bytes, cudaMemcpyHostToDevice, st));
+  GP_OK_OR_RETURN(gp_inverse(g, kern, in_dev, out_dev, ws, ws_bytes, cuda_stream));
+  GP_CUDA_OK(cudaMemcpyAsync(xi_host, out_dev, bytes, cudaMemcpyDeviceToHost, st));
+  return GP_OK;
+}
+
+gp_status gp_check_errors(void* ws, int64_t* n_bad_points) {
+  if (!ws || !n_bad_points) return GP_ERR_INVALID_ARG;
+  Control h;
+  GP_CUDA_OK(cudaMemcpy(&h, ws, sizeof(Control), cudaMemcpyDeviceToHost));
+  *n_bad_points = (int64_t)h.n_bad;
+  if (h.timeout) return GP_ERR_CUDA;
+  return h.n_bad ? GP_ERR_NOT_PD : GP_OK;
+}
+
+const char* gp_status_string(gp_status s) {
+  switch (s) {
+    case GP_OK: return "ok";
+    case GP_ERR_INVALID_ARG: return "invalid argument";
+    case GP_ERR_UNSUPPORTED: return "unsupported (k, d, dtype) or size";
+    case GP_ERR_NOT_PD: return "a conditional covariance was not positive definite";
+    case GP_ERR_CUDA: return "CUDA error or no CUDA device";
+    case GP_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+  }
+  return "unknown status";
+}
+
+int32_t gp_has_specialised(int32_t dtype, int32_t k, int32_t d, int32_t kind) {
+  return has_specialised(dtype, k, d, kind) ? 1 : 0;
+}
+
+int64_t gp_launch_count(void) { return (int64_t)g_launches.load(std::memory_order_relaxed); }
+
+}  // extern "C"

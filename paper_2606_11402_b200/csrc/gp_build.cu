@@ -1,0 +1,314 @@
+// Plain GPU graph builder.  Separately timed.
+//
+//   b1 order   bit-reversed left-balanced k-d tree: node i at level l = floor(log2(i+1)),
+//              position p = i - (2^l - 1), children i + 2^l (left) and i + 2^(l+1) (right).  Built level
+//              by level: one global radix sort per level by (subtree id, rank of the point along
+//              dimension l mod d); the element at offset S(left child) of its subtree becomes the node.
+//              Ranks are dense (coordinate, user id) ranks, so ties are broken by user id (R-4).
+//   b2 kNN     per query i: depth-first walk of the tree restricted to nodes < i (every prefix of the
+//              order is itself a valid tree), candidates ranked by (fp64 FMA-free squared
+//              distance, tree index) (R-5).  One thread per query, queries of one warp are
+//              spatial neighbours (heap-order enumeration of each level).
+//   b3 depth   d_i = 1 + max_{j in c(i)} d_j by in-place parallel sweeps until nothing changes.
+//   b4 sort    stable sort of tree indices by depth (optionally by Morton code inside a depth), remap.
+//
+// Sorting and scanning use CUB (a library primitive on a path that is not the hot path).
+#include <cub/device/device_radix_sort.cuh>
+
+#include "gp_common.cuh"
+
+namespace gp {
+
+struct BuildLayout {
+  size_t ctrl, rank, keys_a, keys_b, vals_a, vals_b, seg, perm_tree, x_tree, nbr_tree, depth_tree, tree2pos,
+      pos2tree, bbox, boff, cub_tmp, cub_bytes, total;
+};
+
+static BuildLayout build_layout(int64_t n, int d, int k, int dtype) {
+  BuildLayout L{};
+  size_t B = dtype_bytes(dtype), N = (size_t)n, off = 0;
+  auto take = [&](size_t bytes) { size_t o = off; off += align_up(bytes, 256); return o; };
+  L.ctrl = take(kCtrlBytes);
+  L.rank = take(N * 4 * d);
+  L.keys_a = take(N * 8);
+  L.keys_b = take(N * 8);
+  L.vals_a = take(N * 4);
+  L.vals_b = take(N * 4);
+  L.seg = take(N * 4);
+  L.perm_tree = take(N * 4);
+  L.x_tree = take(N * d * B);
+  L.nbr_tree = take(N * (size_t)k * 4);
+  L.depth_tree = take(N * 4);
+  L.tree2pos = take(N * 4);
+  L.pos2tree = take(N * 4);
+  L.bbox = take(256);
+  L.boff = take(((size_t)kMaxBatches + 2) * 8);
+  L.cub_bytes = (64u << 20) + N / 2;
+  L.cub_tmp = take(L.cub_bytes);
+  L.total = off;
+  return L;
+}
+
+// ---- small helpers ---------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t order_bits(float f) {
+  f += 0.0f;  // -0 -> +0
+  uint32_t u = __float_as_uint(f);
+  return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ uint64_t order_bits(double f) {
+  f += 0.0;
+  uint64_t u = (uint64_t)__double_as_longlong(f);
+  return (u & 0x8000000000000000ULL) ? ~u : (u | 0x8000000000000000ULL);
+}
+
+template <typename T, typename KeyT>
+__global__ void coord_keys_kernel(const T* __restrict__ x, int64_t n, int d, int dim, KeyT* __restrict__ keys,
+                                  uint32_t* __restrict__ ids) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  keys[i] = (KeyT)order_bits(x[i * d + dim]);
+  ids[i] = (uint32_t)i;
+}
+
+__global__ void scatter_rank_kernel(const uint32_t* __restrict__ sorted_ids, int64_t n, uint32_t* __restrict__ rank) {
+  int64_t p = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < n) rank[sorted_ids[p]] = (uint32_t)p;
+}
+
+__global__ void iota_seg_kernel(uint32_t* __restrict__ ids, uint32_t* __restrict__ seg, int64_t n) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) { ids[i] = (uint32_t)i; seg[i] = 0u; }
+}
+
+__global__ void level_keys_kernel(const uint32_t* __restrict__ ids, const uint32_t* __restrict__ seg,
+                                  const uint32_t* __restrict__ rank_dim, int64_t m, int rank_bits,
+                                  uint64_t* __restrict__ keys) {
+  int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e < m) keys[e] = ((uint64_t)seg[e] << rank_bits) | (uint64_t)rank_dim[ids[e]];
+}
+
+// Tree shape of an N-node prefix (R-2): levels 0..Lam-1 full, level Lam holds positions 0..mlast-1.
+struct TreeShape {
+  int64_t n;
+  int lam;        // level of node n-1
+  int64_t mlast;  // nodes on the last level
+};
+__host__ __device__ inline TreeShape tree_shape(int64_t n) {
+  TreeShape s; s.n = n; int l = 0;
+  while (((int64_t)1 << (l + 1)) - 1 < n) ++l;   // smallest l with 2^(l+1) - 1 >= n
+  s.lam = l; s.mlast = n - (((int64_t)1 << l) - 1);
+  return s;
+}
+// nodes of the last level lying in the subtree rooted at (l, p): positions q < mlast with q mod 2^l == p
+__host__ __device__ inline int64_t last_level_in(const TreeShape& s, int l, int64_t p) {
+  int64_t step = (int64_t)1 << l;
+  return p < s.mlast ? (s.mlast - p + step - 1) / step : 0;
+}
+__host__ __device__ inline int64_t subtree_size(const TreeShape& s, int l, int64_t p) {
+  if (l > s.lam) return 0;
+  if (l == s.lam) return p < s.mlast ? 1 : 0;
+  return (((int64_t)1 << (s.lam - l)) - 1) + last_level_in(s, l, p);
+}
+// elements in subtrees (l, 0..p-1)
+__host__ __device__ inline int64_t subtree_prefix(const TreeShape& s, int l, int64_t p) {
+  int64_t step = (int64_t)1 << l;
+  int64_t last = (s.mlast / step) * p + (s.mlast % step < p ? s.mlast % step : p);
+  if (l == s.lam) return last;
+  return p * (((int64_t)1 << (s.lam - l)) - 1) + last;
+}
+
+// After the level-l sort: element e of subtree (l, p) at offset q inside it goes left (q < S_left), becomes
+// node (l, p) (q == S_left) or goes right.
+__global__ void level_split_kernel(const uint64_t* __restrict__ keys, const uint32_t* __restrict__ ids,
+                                   int64_t m, int rank_bits, int l, TreeShape shape, uint32_t* __restrict__ seg_out,
+                                   uint32_t* __restrict__ perm_tree) {
+  int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= m) return;
+  int64_t p = (int64_t)(keys[e] >> rank_bits);
+  int64_t q = e - subtree_prefix(shape, l, p);
+  int64_t sl = subtree_size(shape, l + 1, p);
+  uint32_t out;
+  if (q < sl) out = (uint32_t)p;
+  else if (q == sl) { perm_tree[(((int64_t)1 << l) - 1) + p] = ids[e]; out = (uint32_t)((int64_t)2 << l); }  // retired
+  else out = (uint32_t)(p + ((int64_t)1 << l));
+  seg_out[e] = out;
+}
+
+template <typename T>
+__global__ void gather_points_kernel(const T* __restrict__ x_src, const uint32_t* __restrict__ idx, int64_t n, int d,
+                                     T* __restrict__ x_dst) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  int64_t s = idx[i];
+  for (int t = 0; t < d; ++t) x_dst[i * d + t] = x_src[s * d + t];
+}
+
+// ---- b2: preceding kNN --------------------------------------------------------------------------------
+// canonical squared distance (R-5): double, left-to-right, no FMA contraction
+template <typename T>
+__device__ __forceinline__ double d2_canon(const double* xi, const T* __restrict__ xj, int d) {
+  double acc = 0.0;
+  for (int t = 0; t < d; ++t) {
+    double dx = __dsub_rn(xi[t], (double)xj[t]);
+    double sq = __dmul_rn(dx, dx);
+    acc = t == 0 ? sq : __dadd_rn(acc, sq);
+  }
+  return acc;
+}
+
+template <typename T, int KMAX>
+__global__ void __launch_bounds__(128)
+knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int32_t* __restrict__ nbr) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  // thread t -> level l, heap position q -> bit-reversed position p -> tree index i: the queries of one
+  // warp are consecutive leaves of the same level, i.e. spatial neighbours
+  int l = 63 - __clzll((unsigned long long)(t + 1));
+  int64_t q = t - (((int64_t)1 << l) - 1);
+  int64_t p = l == 0 ? 0 : (int64_t)(__brevll((unsigned long long)q) >> (64 - l));
+  int64_t i = (((int64_t)1 << l) - 1) + p;
+  if (i >= n || i < n0) return;
+
+  double xi[kMaxD];
+  for (int a = 0; a < d; ++a) xi[a] = (double)x[i * d + a];
+  double bd[KMAX];
+  int32_t bi[KMAX];
+  int cnt = 0, worst = 0;
+  double wd = 0.0; int32_t wi = -1;
+
+  struct Ent { int32_t node; double pd2; };
+  Ent stack[40];
+  int sp = 0;
+  stack[sp++] = {0, 0.0};
+  while (sp > 0) {
+    Ent e = stack[--sp];
+    if (cnt == k && e.pd2 > wd) continue;
+    int32_t j = e.node;
+    double dj = d2_canon<T>(xi, x + (int64_t)j * d, d);
+    if (cnt < k) {
+      bd[cnt] = dj; bi[cnt] = j; ++cnt;
+      if (cnt == k) {
+        worst = 0;
+        for (int a = 1; a < k; ++a)
+          if (bd[a] > bd[worst] || (bd[a] == bd[worst] && bi[a] > bi[worst])) worst = a;
+        wd = bd[worst]; wi = bi[worst];
+      }
+    } else if (dj < wd || (dj == wd && j < wi)) {
+      bd[worst] = dj; bi[worst] = j;
+      worst = 0;
+      for (int a = 1; a < k; ++a)
+        if (bd[a] > bd[worst] || (bd[a] == bd[worst] && bi[a] > bi[worst])) worst = a;
+      wd = bd[worst]; wi = bi[worst];
+    }
+    int lj = 31 - __clz(j + 1);
+    int dim = lj % d;
+    double diff = __dsub_rn(xi[dim], (double)x[(int64_t)j * d + dim]);
+    int64_t left = (int64_t)j + ((int64_t)1 << lj), right = (int64_t)j + ((int64_t)2 << lj);
+    int64_t near = diff < 0.0 ? left : right, far = diff < 0.0 ? right : left;
+    double plane = __dmul_rn(diff, diff);
+    if (far < i && sp < 40) stack[sp++] = {(int32_t)far, plane > e.pd2 ? plane : e.pd2};
+    if (near < i && sp < 40) stack[sp++] = {(int32_t)near, e.pd2};
+  }
+  // nearest first (selection sort on (d2, index))
+  int32_t* out = nbr + (i - n0) * k;
+  for (int a = 0; a < k; ++a) {
+    int best = a;
+    for (int b = a + 1; b < k; ++b)
+      if (bd[b] < bd[best] || (bd[b] == bd[best] && bi[b] < bi[best])) best = b;
+    double td = bd[a]; bd[a] = bd[best]; bd[best] = td;
+    int32_t ti = bi[a]; bi[a] = bi[best]; bi[best] = ti;
+    out[a] = bi[a];
+  }
+}
+
+// ---- b3: depth ----------------------------------------------------------------------------------------
+__global__ void depth_sweep_kernel(const int32_t* __restrict__ nbr, int64_t n, int64_t n0, int k,
+                                   int32_t* depth, unsigned int* changed) {
+  int64_t i = n0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int32_t* row = nbr + (i - n0) * k;
+  int32_t m = 0;
+  for (int a = 0; a < k; ++a) {
+    int32_t dj = ((volatile int32_t*)depth)[row[a]];
+    m = dj > m ? dj : m;
+  }
+  int32_t nd = m + 1;
+  if (((volatile int32_t*)depth)[i] != nd) { ((volatile int32_t*)depth)[i] = nd; *changed = 1u; }
+}
+
+// ---- b4: depth sort -----------------------------------------------------------------------------------
+template <typename T>
+__global__ void bbox_kernel(const T* __restrict__ x, int64_t n, int d, unsigned long long* bbox /*[2*kMaxD]*/) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  for (int t = 0; t < d; ++t) {
+    unsigned long long u = order_bits((double)x[i * d + t]);
+    atomicMin(&bbox[2 * t], u);
+    atomicMax(&bbox[2 * t + 1], u);
+  }
+}
+__device__ __forceinline__ double unorder_bits(unsigned long long u) {
+  u = (u & 0x8000000000000000ULL) ? (u & 0x7fffffffffffffffULL) : ~u;
+  return __longlong_as_double((long long)u);
+}
+
+template <typename T>
+__global__ void sort_keys_kernel(const T* __restrict__ x_tree, const int32_t* __restrict__ depth, int64_t n,
+                                 int64_t n0, int d, int spatial, int cell_bits, int depth_shift,
+                                 const unsigned long long* __restrict__ bbox, uint64_t* __restrict__ keys,
+                                 uint32_t* __restrict__ vals) {
+  int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= n - n0) return;
+  int64_t i = n0 + e;
+  uint64_t code = 0;
+  if (spatial) {
+    uint32_t cell[kMaxD];
+    for (int t = 0; t < d; ++t) {
+      double lo = unorder_bits(bbox[2 * t]), hi = unorder_bits(bbox[2 * t + 1]);
+      double w = hi > lo ? hi - lo : 1.0;
+      double f = ((double)x_tree[i * d + t] - lo) / w * (double)((uint64_t)1 << cell_bits);
+      uint64_t c = f <= 0.0 ? 0 : (uint64_t)f;
+      uint64_t cmax = ((uint64_t)1 << cell_bits) - 1;
+      cell[t] = (uint32_t)(c > cmax ? cmax : c);
+    }
+    for (int b = 0; b < cell_bits; ++b)
+      for (int t = 0; t < d; ++t) code |= (uint64_t)((cell[t] >> b) & 1u) << (b * d + t);
+  }
+  keys[e] = ((uint64_t)depth[i] << depth_shift) | code;
+  vals[e] = (uint32_t)i;
+}
+
+__global__ void positions_kernel(const uint32_t* __restrict__ sorted_tree, int64_t n, int64_t n0,
+                                 uint32_t* __restrict__ pos2tree, uint32_t* __restrict__ tree2pos) {
+  int64_t pos = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (pos >= n) return;
+  uint32_t t = pos < n0 ? (uint32_t)pos : sorted_tree[pos - n0];
+  pos2tree[pos] = t;
+  tree2pos[t] = (uint32_t)pos;
+}
+
+template <typename T>
+__global__ void emit_graph_kernel(const uint32_t* __restrict__ pos2tree, const uint32_t* __restrict__ tree2pos,
+                                  const uint32_t* __restrict__ perm_tree, const T* __restrict__ x_tree,
+                                  const int32_t* __restrict__ depth_tree, const int32_t* __restrict__ nbr_tree,
+                                  int64_t n, int64_t n0, int d, int k, int64_t* __restrict__ perm,
+                                  T* __restrict__ x_graph, int32_t* __restrict__ depth, int32_t* __restrict__ nbr,
+                                  int64_t* __restrict__ boff) {
+  int64_t pos = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (pos >= n) return;
+  int64_t t = pos2tree[pos];
+  perm[pos] = (int64_t)perm_tree[t];
+  for (int a = 0; a < d; ++a) x_graph[pos * d + a] = x_tree[t * d + a];
+  int32_t dep = depth_tree[t];
+  depth[pos] = dep;
+  if (pos >= n0) {
+    const int32_t* src = nbr_tree + (t - n0) * k;
+    int32_t* dst = nbr + (pos - n0) * k;
+    for (int a = 0; a < k; ++a) dst[a] = (int32_t)tree2pos[src[a]];
+    int32_t prev = pos == n0 ? 0 : depth_tree[pos2tree[pos - 1]];
+    if (dep != prev) boff[dep - 1] = pos;       // first position of batch `dep` (depths are contiguous from 1)
+    if (pos == n - 1) boff[dep] = n;
+  }
+}
+
+}  // namespace gp

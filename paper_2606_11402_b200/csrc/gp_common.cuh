@@ -1,0 +1,222 @@
+// Shared device/host definitions for the GraphGP sm_100a kernels.
+// Nothing here is shared with oracle/ (which has its own, independent arithmetic).
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/graphgp.h"
+
+namespace gp {
+
+constexpr int kMaxK = 64;
+constexpr int kMaxD = 4;
+constexpr int kCtrlBytes = 512;
+constexpr int kMaxBatches = 1 << 20;
+
+// First kCtrlBytes of every workspace; zeroed by the library at the start of each op.
+struct Control {
+  unsigned long long n_bad;    // points whose conditional was not positive definite
+  unsigned long long ticket;   // dataflow forward: next chunk to hand out
+  unsigned long long timeout;  // dataflow watchdog fired (a bug, never expected)
+  unsigned long long pad0;
+  double acc[8];               // [0] logdet  [1] dlogdet/dsigma  [2] dlogdet/dell  [3] theta_bar sigma  [4] theta_bar ell
+  double build_ms[4];          // graph builder stage times
+  unsigned long long pad[4];
+};
+static_assert(sizeof(Control) <= kCtrlBytes, "control block");
+
+// Packed per-point record the register-resident kernels gather: coordinates (d <= 3, unused slots 0)
+// and the point's value in ONE aligned 4-scalar record, so a neighbour costs one 16 B (fp32) / 32 B
+// (fp64) load = one L2 sector, instead of d+1 scattered 4 B loads.
+template <typename T> struct alignas(4 * sizeof(T)) Rec { T x0, x1, x2, v; };
+
+// Kernel parameters in the working precision, unit-sigma form:  K/sigma^2 = rho + eps*delta.
+// q = qscale * |x_a - x_b|^2 is the argument the correlation needs (see rho_from_q); the difference
+// is taken on the RAW coordinates (exact for nearby points), the scale applied afterwards.
+template <typename T>
+struct KParams {
+  T qscale;  // fp32 (base-2 exponent): SE log2e/(2 ell^2); Matern-3/2 3 log2e^2/ell^2; EXP log2e^2/ell^2
+             // fp64 (natural exponent): SE 1/(2 ell^2);   Matern-3/2 3/ell^2;          EXP 1/ell^2
+  T eps;     // relative jitter
+  T sigma;
+  T diag;    // 1 + eps
+  T inv_ell;
+};
+
+template <typename T> __host__ inline KParams<T> make_kparams(const gp_kernel& k);
+template <> __host__ inline KParams<float> make_kparams<float>(const gp_kernel& k) {
+  const double log2e = 1.4426950408889634074;
+  KParams<float> p;
+  double s = 0;
+  switch (k.kind) {
+    case GP_KERNEL_SE: s = 0.5 * log2e / (k.ell * k.ell); break;
+    case GP_KERNEL_MATERN32: s = 3.0 * log2e * log2e / (k.ell * k.ell); break;
+    default: s = log2e * log2e / (k.ell * k.ell); break;
+  }
+  p.qscale = (float)s; p.eps = (float)k.jitter; p.sigma = (float)k.sigma; p.diag = (float)(1.0 + k.jitter);
+  p.inv_ell = (float)(1.0 / k.ell);
+  return p;
+}
+template <> __host__ inline KParams<double> make_kparams<double>(const gp_kernel& k) {
+  KParams<double> p;
+  double s = 0;
+  switch (k.kind) {
+    case GP_KERNEL_SE: s = 0.5 / (k.ell * k.ell); break;
+    case GP_KERNEL_MATERN32: s = 3.0 / (k.ell * k.ell); break;
+    default: s = 1.0 / (k.ell * k.ell); break;
+  }
+  p.qscale = s; p.eps = k.jitter; p.sigma = k.sigma; p.diag = 1.0 + k.jitter; p.inv_ell = 1.0 / k.ell;
+  return p;
+}
+
+// ---- per-precision math -------------------------------------------------------------------------
+template <typename T> struct Math;
+template <> struct Math<float> {
+  static __device__ __forceinline__ float rsqrt_approx(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+  // MUFU.RSQ (about 2 ulp) + one Newton step: error well below the fp32 rounding of the factor itself
+  static __device__ __forceinline__ float rsqrt(float x) {
+    float y = rsqrt_approx(x);
+    float h = 0.5f * y;
+    float e = fmaf(-x * y, h, 0.5f);   // 0.5 - 0.5 x y^2
+    return fmaf(y, e, y);
+  }
+  static __device__ __forceinline__ float sqrt_approx(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+  static __device__ __forceinline__ float sqrt(float x) { return sqrtf(x); }
+  static __device__ __forceinline__ float ex2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+  static __device__ __forceinline__ float fma(float a, float b, float c) { return fmaf(a, b, c); }
+  static __device__ __forceinline__ float log(float x) { return logf(x); }
+  static __device__ __forceinline__ float fmin(float a, float b) { return fminf(a, b); }
+  // rho as a function of q = qscale * |x_a - x_b|^2 (base-2 exponent folded in).
+  template <int KIND> static __device__ __forceinline__ float rho_from_q(float q) {
+    if (KIND == GP_KERNEL_SE) return ex2(-q);
+    float t = sqrt_approx(q);                            // MUFU.SQRT: sqrt(0) = 0, no guard needed
+    if (KIND == GP_KERNEL_MATERN32) return fmaf(t, 0.69314718055994530942f, 1.0f) * ex2(-t);
+    return ex2(-t);
+  }
+  // ell * d rho / d ell  as a function of q (dimensionless; the caller divides by ell).
+  template <int KIND> static __device__ __forceinline__ float drho_from_q(float q) {
+    const float ln2 = 0.69314718055994530942f;
+    if (KIND == GP_KERNEL_SE) return 2.0f * ln2 * q * ex2(-q);            // rho * r^2/ell^2
+    float t = sqrt_approx(q);
+    if (KIND == GP_KERNEL_MATERN32) { float a = t * ln2; return a * a * ex2(-t); }   // a^2 e^-a
+    return t * ln2 * ex2(-t);                                               // rho * r/ell
+  }
+};
+template <> struct Math<double> {
+  static __device__ __forceinline__ double rsqrt(double x) { return 1.0 / ::sqrt(x); }
+  static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
+  static __device__ __forceinline__ double fma(double a, double b, double c) { return ::fma(a, b, c); }
+  static __device__ __forceinline__ double log(double x) { return ::log(x); }
+  static __device__ __forceinline__ double fmin(double a, double b) { return ::fmin(a, b); }
+  template <int KIND> static __device__ __forceinline__ double rho_from_q(double q) {
+    if (KIND == GP_KERNEL_SE) return ::exp(-q);
+    double a = ::sqrt(q);
+    if (KIND == GP_KERNEL_MATERN32) return (1.0 + a) * ::exp(-a);
+    return ::exp(-a);
+  }
+  template <int KIND> static __device__ __forceinline__ double drho_from_q(double q) {
+    if (KIND == GP_KERNEL_SE) return 2.0 * q * ::exp(-q);
+    double a = ::sqrt(q);
+    if (KIND == GP_KERNEL_MATERN32) return a * a * ::exp(-a);
+    return a * ::exp(-a);
+  }
+};
+
+// runtime-kind versions (generic kernel, dense head)
+template <typename T> __device__ __forceinline__ T rho_rt(int kind, T q) {
+  switch (kind) {
+    case GP_KERNEL_SE: return Math<T>::template rho_from_q<GP_KERNEL_SE>(q);
+    case GP_KERNEL_MATERN32: return Math<T>::template rho_from_q<GP_KERNEL_MATERN32>(q);
+    default: return Math<T>::template rho_from_q<GP_KERNEL_EXP>(q);
+  }
+}
+template <typename T> __device__ __forceinline__ T drho_rt(int kind, T q) {
+  switch (kind) {
+    case GP_KERNEL_SE: return Math<T>::template drho_from_q<GP_KERNEL_SE>(q);
+    case GP_KERNEL_MATERN32: return Math<T>::template drho_from_q<GP_KERNEL_MATERN32>(q);
+    default: return Math<T>::template drho_from_q<GP_KERNEL_EXP>(q);
+  }
+}
+
+// ---- host-side helpers ---------------------------------------------------------------------------
+void count_launch(int n = 1);
+
+#define GP_CUDA_OK(expr)                                   \
+  do {                                                     \
+    cudaError_t e__ = (expr);                              \
+    if (e__ != cudaSuccess) return GP_ERR_CUDA;            \
+  } while (0)
+#define GP_OK_OR_RETURN(expr)                              \
+  do {                                                     \
+    gp_status s__ = (expr);                                \
+    if (s__ != GP_OK) return s__;                          \
+  } while (0)
+#define GP_LAUNCH_CHECK()                                  \
+  do {                                                     \
+    gp::count_launch();                                    \
+    if (cudaGetLastError() != cudaSuccess) return GP_ERR_CUDA; \
+  } while (0)
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+inline size_t dtype_bytes(int dtype) { return dtype == GP_F64 ? 8 : 4; }
+
+// Workspace layout (byte offsets from ws).  The head is always factored in fp64.
+//   ctrl     Control
+//   boff     device copy of batch_off (int64 [n_batches + 1]) + chunk prefix (int64 [n_batches + 1])
+//   head     (n0 + carried) x n0 doubles: factor of K_head/sigma^2 + carried rows
+//   rec      packed records Rec<T>[n]                          (register-resident kernels only)
+//   g        VJP: running cotangent, T[n]
+struct WsLayout {
+  size_t ctrl_off, boff_off, head_off, rec_off, g_off, total;
+  size_t head_rows;
+};
+inline WsLayout ws_layout(const gp_graph* g, int op) {
+  WsLayout w{};
+  size_t B = dtype_bytes(g->dtype);
+  size_t n0 = (size_t)g->n0, n = (size_t)g->n;
+  size_t off = 0;
+  w.ctrl_off = off; off += kCtrlBytes;
+  w.boff_off = off; off += align_up(2 * ((size_t)g->n_batches + 1) * sizeof(int64_t), 256);
+  size_t carried = (op == GP_OP_INVERSE) ? 1 : (op == GP_OP_VJP ? n0 : 0);
+  w.head_rows = n0 + carried;
+  size_t head_elems = w.head_rows * n0;
+  if (op == GP_OP_VJP) head_elems += 2 * n0 * n0;  // scratch for L^T Lbar and the K_bar products
+  w.head_off = off; off += align_up(head_elems * sizeof(double), 256);
+  w.rec_off = off; off += align_up(n * 4 * B, 256);
+  w.g_off = off;
+  if (op == GP_OP_VJP) off += align_up(n * B, 256);
+  w.total = off;
+  return w;
+}
+
+struct OpCtx {
+  const gp_graph* g;
+  const gp_kernel* kern;
+  char* ws;
+  WsLayout lay;
+  cudaStream_t st;
+  Control* ctrl() const { return (Control*)(ws + lay.ctrl_off); }
+  int64_t* boff_dev() const { return (int64_t*)(ws + lay.boff_off); }
+  double* head() const { return (double*)(ws + lay.head_off); }
+  void* rec() const { return ws + lay.rec_off; }
+  void* gbar() const { return ws + lay.g_off; }
+};
+
+// ---- entry points implemented across the .cu files ------------------------------------------------
+// dense head (gp_head.cu)
+gp_status head_factor(const OpCtx& c, const void* carried_src /*dtype [n0] or null*/, int n_carried);
+gp_status head_forward(const OpCtx& c, const void* xi, void* v, void* rec, bool rec_is_packed);
+gp_status head_inverse_out(const OpCtx& c, void* xi);
+gp_status head_logdet(const OpCtx& c, double* acc /*device: acc[0] += logdet head*/, double* grad_acc);
+gp_status head_vjp(const OpCtx& c, const void* xi, const void* gbar, void* xibar, double* acc);
+
+// conditioning (gp_ops.cu, gp_vjp.cu)
+gp_status run_forward(const OpCtx& c, const void* xi, void* v);
+gp_status run_inverse(const OpCtx& c, const void* v, void* xi);
+gp_status run_logdet(const OpCtx& c, double* logdet, double* grad);
+gp_status run_vjp(const OpCtx& c, const void* xi, const void* v, const void* vbar, void* xibar, double* thetabar);
+bool has_specialised(int dtype, int k, int d, int kind);
+
+}  // namespace gp

@@ -1,0 +1,257 @@
+// Dense initial block (Alg. 1 line 1): the first n0 values come from a dense
+// Cholesky of K_head.  Always factored in fp64 (n0^3/3 flops are negligible next to the N k^3 of the
+// conditioning, and the head feeds every later point), whatever the working dtype.
+//
+// Right-looking blocked Cholesky of M = K_head / sigma^2 (row-major, lower part), NB = 32, with
+// `carried` extra rows below the square part that receive the same panel solves and trailing updates:
+// a carried row that starts as r^T ends as (L^-1 r)^T, exactly the values row of Alg. 1.
+//   inverse : 1 carried row  = v_head^T      ->  (L^-1 v_head)^T = sigma * xi_head^T
+//   VJP     : n0 carried rows = identity     ->  L^-T
+#include "gp_cond.cuh"
+
+namespace gp {
+
+constexpr int NB = 32;
+
+template <typename T>
+__global__ void head_build_kernel(const T* __restrict__ x, int d, int n0, int kind, KParams<double> kp,
+                                  double* __restrict__ A) {
+  int c = blockIdx.x * blockDim.x + threadIdx.x;
+  int r = blockIdx.y * blockDim.y + threadIdx.y;
+  if (r >= n0 || c > r) return;
+  double val;
+  if (r == c) {
+    val = kp.diag;
+  } else {
+    double d2 = 0.0;
+    for (int t = 0; t < d; ++t) {
+      double dx = (double)x[(size_t)r * d + t] - (double)x[(size_t)c * d + t];
+      d2 = fma(dx, dx, d2);
+    }
+    val = rho_rt<double>(kind, d2 * kp.qscale);
+  }
+  A[(size_t)r * n0 + c] = val;
+}
+
+// carried rows: mode 1 = one row holding src[0:n0]; mode 2 = identity (n0 rows)
+template <typename T>
+__global__ void head_carry_init_kernel(const T* __restrict__ src, int n0, int mode, double* __restrict__ A) {
+  int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int64_t total = mode == 1 ? n0 : (int64_t)n0 * n0;
+  if (e >= total) return;
+  double* C = A + (size_t)n0 * n0;
+  if (mode == 1) C[e] = (double)src[e];
+  else C[e] = (e / n0 == e % n0) ? 1.0 : 0.0;
+}
+
+// One block column: every CTA factors the nb x nb diagonal block in shared memory (redundantly — it is
+// tiny), CTA 0 writes it back, and each thread then solves one row of the panel below against it.
+__global__ void __launch_bounds__(64)
+head_panel_kernel(double* __restrict__ A, int n0, int rows_total, int j0, Control* ctrl) {
+  __shared__ double Ds[NB][NB + 1];
+  __shared__ double invd[NB];
+  const int nb = min(NB, n0 - j0);
+  const int tid = threadIdx.x;
+  for (int e = tid; e < NB * NB; e += blockDim.x) {
+    int r = e / NB, c = e % NB;
+    Ds[r][c] = (r < nb && c <= r) ? A[(size_t)(j0 + r) * n0 + j0 + c] : (r == c ? 1.0 : 0.0);
+  }
+  __syncthreads();
+  if (tid < 32) {
+    const int lane = tid;
+    for (int j = 0; j < nb; ++j) {
+      if (lane == j) {
+        double piv = Ds[j][j];
+        if (!(piv > 0.0) && blockIdx.x == 0) atomicAdd(&ctrl->n_bad, 1ULL);
+        double sq = sqrt(piv);
+        Ds[j][j] = sq;
+        invd[j] = 1.0 / sq;
+      }
+      __syncwarp();
+      if (lane > j && lane < nb) {
+        double l = Ds[lane][j] * invd[j];
+        Ds[lane][j] = l;
+      }
+      __syncwarp();
+      if (lane > j && lane < nb) {
+        double l = Ds[lane][j];
+        for (int c = j + 1; c <= lane; ++c) Ds[lane][c] = fma(-l, Ds[c][j], Ds[lane][c]);
+      }
+      __syncwarp();
+    }
+  }
+  __syncthreads();
+  if (blockIdx.x == 0) {
+    for (int e = tid; e < nb * nb; e += blockDim.x) {
+      int r = e / nb, c = e % nb;
+      if (c <= r) A[(size_t)(j0 + r) * n0 + j0 + c] = Ds[r][c];
+    }
+  }
+  int r = j0 + nb + blockIdx.x * blockDim.x + tid;
+  if (r >= rows_total) return;
+  double* arow = A + (size_t)r * n0 + j0;
+  double a[NB];
+#pragma unroll
+  for (int c = 0; c < NB; ++c) a[c] = (c < nb) ? arow[c] : 0.0;
+#pragma unroll
+  for (int c = 0; c < NB; ++c) {
+    double acc = a[c];
+#pragma unroll
+    for (int t = 0; t < c; ++t) acc = fma(-a[t], Ds[c][t], acc);
+    a[c] = (c < nb) ? acc * invd[c] : 0.0;
+  }
+#pragma unroll
+  for (int c = 0; c < NB; ++c)
+    if (c < nb) arow[c] = a[c];
+}
+
+// Trailing update  A[r][c] -= sum_t P[r][t] P[c][t]  for r >= j1 = j0 + nb, j1 <= c <= min(r, n0 - 1).
+__global__ void __launch_bounds__(256)
+head_update_kernel(double* __restrict__ A, int n0, int rows_total, int j0, int nb) {
+  __shared__ double Pr[NB][64 + 2];
+  __shared__ double Pc[NB][64 + 2];
+  const int j1 = j0 + nb;
+  const int r0 = j1 + blockIdx.y * 64, c0 = j1 + blockIdx.x * 64;
+  if (c0 >= n0 || r0 >= rows_total) return;
+  if (r0 < n0 && c0 > r0 + 63) return;   // tile entirely above the diagonal of the square part
+  const int tid = threadIdx.x;
+  for (int e = tid; e < 64 * NB; e += 256) {
+    int row = e / NB, t = e % NB;
+    int rr = r0 + row, cc = c0 + row;
+    Pr[t][row] = (rr < rows_total && t < nb) ? A[(size_t)rr * n0 + j0 + t] : 0.0;
+    Pc[t][row] = (cc < n0 && t < nb) ? A[(size_t)cc * n0 + j0 + t] : 0.0;
+  }
+  __syncthreads();
+  const int tx = tid % 16, ty = tid / 16;
+  double acc[4][4];
+#pragma unroll
+  for (int a = 0; a < 4; ++a)
+#pragma unroll
+    for (int b = 0; b < 4; ++b) acc[a][b] = 0.0;
+#pragma unroll 8
+  for (int t = 0; t < NB; ++t) {
+    double pr[4], pc[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) { pr[a] = Pr[t][ty * 4 + a]; pc[a] = Pc[t][tx * 4 + a]; }
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) acc[a][b] = fma(pr[a], pc[b], acc[a][b]);
+  }
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    int r = r0 + ty * 4 + a;
+    if (r >= rows_total) continue;
+#pragma unroll
+    for (int b = 0; b < 4; ++b) {
+      int c = c0 + tx * 4 + b;
+      if (c >= n0 || (r < n0 && c > r)) continue;
+      A[(size_t)r * n0 + c] -= acc[a][b];
+    }
+  }
+}
+
+gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried) {
+  const int n0 = (int)c.g->n0;
+  if (n0 <= 0) return GP_OK;
+  double* A = c.head();
+  KParams<double> kp = make_kparams<double>(*c.kern);
+  dim3 bb(16, 16), bg((n0 + 15) / 16, (n0 + 15) / 16);
+  if (c.g->dtype == GP_F64)
+    head_build_kernel<double><<<bg, bb, 0, c.st>>>((const double*)c.g->x, c.g->d, n0, c.kern->kind, kp, A);
+  else
+    head_build_kernel<float><<<bg, bb, 0, c.st>>>((const float*)c.g->x, c.g->d, n0, c.kern->kind, kp, A);
+  GP_LAUNCH_CHECK();
+  if (n_carried > 0) {
+    int mode = n_carried == 1 ? 1 : 2;
+    int64_t total = mode == 1 ? n0 : (int64_t)n0 * n0;
+    unsigned grid = (unsigned)((total + 255) / 256);
+    if (c.g->dtype == GP_F64)
+      head_carry_init_kernel<double><<<grid, 256, 0, c.st>>>((const double*)carried_src, n0, mode, A);
+    else
+      head_carry_init_kernel<float><<<grid, 256, 0, c.st>>>((const float*)carried_src, n0, mode, A);
+    GP_LAUNCH_CHECK();
+  }
+  const int rows_total = n0 + n_carried;
+  for (int j0 = 0; j0 < n0; j0 += NB) {
+    int nb = n0 - j0 < NB ? n0 - j0 : NB;
+    int below = rows_total - (j0 + nb);
+    unsigned pg = below > 0 ? (unsigned)((below + 63) / 64) : 1u;
+    head_panel_kernel<<<pg, 64, 0, c.st>>>(A, n0, rows_total, j0, c.ctrl());
+    GP_LAUNCH_CHECK();
+    int cols = n0 - (j0 + nb);
+    if (cols > 0) {
+      dim3 ug((cols + 63) / 64, (below + 63) / 64);
+      head_update_kernel<<<ug, 256, 0, c.st>>>(A, n0, rows_total, j0, nb);
+      GP_LAUNCH_CHECK();
+    }
+  }
+  return GP_OK;
+}
+
+// v_head = sigma * L xi_head  (one warp per row)
+template <typename T>
+__global__ void head_forward_kernel(const double* __restrict__ L, const T* __restrict__ xi, T* __restrict__ v,
+                                    Rec<T>* rec, int n0, double sigma) {
+  int r = blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;
+  int lane = threadIdx.x & 31;
+  if (r >= n0) return;
+  double acc = 0.0;
+  for (int cc = lane; cc <= r; cc += 32) acc = fma(L[(size_t)r * n0 + cc], (double)xi[cc], acc);
+  acc = warp_sum(acc);
+  if (lane == 0) {
+    T out = (T)(sigma * acc);
+    v[r] = out;
+    if (rec) rec[r].v = out;
+  }
+}
+
+gp_status head_forward(const OpCtx& c, const void* xi, void* v, void* rec, bool rec_is_packed) {
+  const int n0 = (int)c.g->n0;
+  if (n0 <= 0) return GP_OK;
+  unsigned grid = (unsigned)((n0 + 3) / 4);
+  if (c.g->dtype == GP_F64)
+    head_forward_kernel<double><<<grid, 128, 0, c.st>>>(c.head(), (const double*)xi, (double*)v,
+                                                      rec_is_packed ? (Rec<double>*)rec : nullptr, n0, c.kern->sigma);
+  else
+    head_forward_kernel<float><<<grid, 128, 0, c.st>>>(c.head(), (const float*)xi, (float*)v,
+                                                     rec_is_packed ? (Rec<float>*)rec : nullptr, n0, c.kern->sigma);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+template <typename T>
+__global__ void head_inverse_out_kernel(const double* __restrict__ carried, T* __restrict__ xi, int n0, double inv_sigma) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n0) xi[i] = (T)(carried[i] * inv_sigma);
+}
+
+gp_status head_inverse_out(const OpCtx& c, void* xi) {
+  const int n0 = (int)c.g->n0;
+  if (n0 <= 0) return GP_OK;
+  const double* carried = c.head() + (size_t)n0 * n0;
+  unsigned grid = (unsigned)((n0 + 255) / 256);
+  if (c.g->dtype == GP_F64)
+    head_inverse_out_kernel<double><<<grid, 256, 0, c.st>>>(carried, (double*)xi, n0, 1.0 / c.kern->sigma);
+  else
+    head_inverse_out_kernel<float><<<grid, 256, 0, c.st>>>(carried, (float*)xi, n0, 1.0 / c.kern->sigma);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+__global__ void head_logdet_kernel(const double* __restrict__ L, int n0, double sigma, double* acc) {
+  __shared__ double red[32];
+  double s = 0.0;
+  for (int j = threadIdx.x; j < n0; j += blockDim.x) s += 2.0 * log(sigma * L[(size_t)j * n0 + j]);
+  block_atomic_add(s, acc, red);
+}
+
+gp_status head_logdet(const OpCtx& c, double* acc, double* /*grad_acc*/) {
+  const int n0 = (int)c.g->n0;
+  if (n0 <= 0) return GP_OK;
+  head_logdet_kernel<<<1, 256, 0, c.st>>>(c.head(), n0, c.kern->sigma, acc);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+}  // namespace gp

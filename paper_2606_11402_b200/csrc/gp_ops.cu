@@ -1,0 +1,240 @@
+// Forward / inverse / logdet kernels of the Vecchia conditioning path.
+//   forward  Alg. 1 lines 2-8: one launch per batch, every point of a batch in parallel
+//   inverse  PAPER.md:91: every point at once
+//   logdet   PAPER.md:9:  sum_i log s_i^2, fp64 accumulation
+#include <type_traits>
+
+#include "gp_cond.cuh"
+
+namespace gp {
+
+enum { OPK_FORWARD = 0, OPK_INVERSE = 1, OPK_LOGDET = 2 };
+constexpr int kCondThreads = 128;
+
+// rec[i] = {x_i, vals_i or 0}
+template <typename T>
+__global__ void pack_kernel(const T* __restrict__ x, const T* __restrict__ vals, Rec<T>* __restrict__ rec,
+                            int64_t n, int d) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  Rec<T> r;
+  r.x0 = x[i * d];
+  r.x1 = d >= 2 ? x[i * d + 1] : T(0);
+  r.x2 = d >= 3 ? x[i * d + 2] : T(0);
+  r.v = vals ? vals[i] : T(0);
+  rec[i] = r;
+}
+
+template <typename T> __device__ __forceinline__ T quiet_nan();
+template <> __device__ __forceinline__ float quiet_nan<float>() { return __int_as_float(0x7fc00000); }
+template <> __device__ __forceinline__ double quiet_nan<double>() { return __longlong_as_double(0x7ff8000000000000LL); }
+
+template <typename T, int K, int D, int KIND, int OP>
+__global__ void __launch_bounds__(kCondThreads)
+cond_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* __restrict__ in,
+            T* __restrict__ out, int64_t start, int64_t end, int64_t n0, KParams<T> kp, Control* ctrl) {
+  __shared__ double red[32];
+  int64_t i = start + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  double ld = 0.0;
+  if (i < end) {
+    Rec<T> self = load_rec<false>(rec + i);
+    Cond<T> c = condition_reg<T, K, D, KIND, false>(rec, nbr + (i - n0) * K, self, kp);
+    T ss = kp.sigma * c.s;
+    if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
+    if (OP == OPK_FORWARD) {
+      T v = Math<T>::fma(ss, in[i], c.m);
+      if (!c.ok) v = quiet_nan<T>();
+      out[i] = v;
+      rec[i].v = v;
+    } else if (OP == OPK_INVERSE) {
+      T xi = (self.v - c.m) / ss;
+      if (!c.ok) xi = quiet_nan<T>();
+      out[i] = xi;
+    } else {
+      ld = c.ok ? 2.0 * (double)Math<T>::log(ss) : 0.0;
+    }
+  }
+  if (OP == OPK_LOGDET) block_atomic_add(ld, &ctrl->acc[0], red);
+}
+
+template <typename T, int OP>
+__global__ void cond_generic_kernel(const T* __restrict__ x, const T* vals, const int32_t* __restrict__ nbr,
+                                    const T* in, T* out, int64_t start, int64_t end, int64_t n0, int d, int k,
+                                    int kind, KParams<T> kp, Control* ctrl, int active) {
+  extern __shared__ double smem_raw[];
+  __shared__ double red[32];
+  int tid = threadIdx.x;
+  int64_t i = start + (int64_t)blockIdx.x * active + tid;
+  double ld = 0.0;
+  if (tid < active && i < end) {
+    Scratch<T> A{reinterpret_cast<T*>(smem_raw) + tid, active};
+    Cond<T> c = condition_generic<T>(x, OP == OPK_LOGDET ? nullptr : vals, d, k, kind, nbr + (i - n0) * k, i, kp, A);
+    T ss = kp.sigma * c.s;
+    if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
+    if (OP == OPK_FORWARD) {
+      T v = Math<T>::fma(ss, in[i], c.m);
+      if (!c.ok) v = quiet_nan<T>();
+      out[i] = v;
+    } else if (OP == OPK_INVERSE) {
+      T xi = (in[i] - c.m) / ss;
+      if (!c.ok) xi = quiet_nan<T>();
+      out[i] = xi;
+    } else {
+      ld = c.ok ? 2.0 * (double)Math<T>::log(ss) : 0.0;
+    }
+  }
+  if (OP == OPK_LOGDET) block_atomic_add(ld, &ctrl->acc[0], red);
+}
+
+// Threads of a generic block that own a scratch column (the block is padded to a multiple of 32).
+int generic_active_threads(int k, size_t elem_bytes, bool with_vjp) {
+  size_t per = (size_t)generic_scratch_elems(k, with_vjp) * elem_bytes;
+  size_t budget = 200 * 1024;
+  size_t a = budget / per;
+  if (a > 128) a = 128;
+  if (a >= 32) a = a / 32 * 32;
+  if (a < 1) a = 1;
+  return (int)a;
+}
+
+// ---- specialisation table ------------------------------------------------------------------------
+// (dtype, K, D) triples with a register-resident kernel; every KIND is instantiated for each.
+#define GP_SPEC_TABLE(X) \
+  X(float, 8, 3) X(float, 16, 3) X(float, 8, 2) X(float, 16, 2) X(double, 8, 3) X(double, 8, 2)
+
+bool has_specialised(int dtype, int k, int d, int kind) {
+  if (kind < 0 || kind > 2) return false;
+#define X(T, K, D) \
+  if ((dtype == GP_F64) == (sizeof(T) == 8) && k == K && d == D) return true;
+  GP_SPEC_TABLE(X)
+#undef X
+  return false;
+}
+
+template <typename T, int K, int D, int OP>
+static gp_status launch_spec_kind(const OpCtx& c, const T* in, T* out, int64_t start, int64_t end) {
+  int64_t cnt = end - start;
+  if (cnt <= 0) return GP_OK;
+  unsigned grid = (unsigned)((cnt + kCondThreads - 1) / kCondThreads);
+  KParams<T> kp = make_kparams<T>(*c.kern);
+  Rec<T>* rec = (Rec<T>*)c.rec();
+  switch (c.kern->kind) {
+    case GP_KERNEL_SE:
+      cond_kernel<T, K, D, GP_KERNEL_SE, OP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, in, out, start, end, c.g->n0, kp, c.ctrl());
+      break;
+    case GP_KERNEL_MATERN32:
+      cond_kernel<T, K, D, GP_KERNEL_MATERN32, OP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, in, out, start, end, c.g->n0, kp, c.ctrl());
+      break;
+    default:
+      cond_kernel<T, K, D, GP_KERNEL_EXP, OP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, in, out, start, end, c.g->n0, kp, c.ctrl());
+      break;
+  }
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+template <typename T, int OP>
+static gp_status launch_generic(const OpCtx& c, const T* vals, const T* in, T* out, int64_t start, int64_t end) {
+  int64_t cnt = end - start;
+  if (cnt <= 0) return GP_OK;
+  int k = c.g->k;
+  int active = generic_active_threads(k, sizeof(T), false);
+  int threads = (active + 31) / 32 * 32;
+  size_t smem = (size_t)generic_scratch_elems(k, false) * sizeof(T) * active;
+  static bool attr_set = false;
+  if (!attr_set) {
+    GP_CUDA_OK(cudaFuncSetAttribute(cond_generic_kernel<T, OP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
+    attr_set = true;
+  }
+  unsigned grid = (unsigned)((cnt + active - 1) / active);
+  KParams<T> kp = make_kparams<T>(*c.kern);
+  cond_generic_kernel<T, OP><<<grid, threads, smem, c.st>>>((const T*)c.g->x, vals, c.g->nbr, in, out, start, end,
+                                                          c.g->n0, c.g->d, k, c.kern->kind, kp, c.ctrl(), active);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+static bool use_spec(const OpCtx& c) {
+  if (c.g->flags & GP_FLAG_GENERIC_KERNEL) return false;
+  if (!has_specialised(c.g->dtype, c.g->k, c.g->d, c.kern->kind)) return false;
+  return (((uintptr_t)c.g->nbr) & 15) == 0;  // vectorised index loads need 16 B alignment
+}
+
+template <typename T, int OP>
+static gp_status launch_range(const OpCtx& c, bool spec, const T* vals, const T* in, T* out, int64_t start, int64_t end) {
+  if (spec) {
+#define X(TT, K, D) \
+    if constexpr (std::is_same<TT, T>::value) {                    \
+      if (c.g->k == K && c.g->d == D) return launch_spec_kind<T, K, D, OP>(c, in, out, start, end); \
+    }
+    GP_SPEC_TABLE(X)
+#undef X
+  }
+  return launch_generic<T, OP>(c, vals, in, out, start, end);
+}
+
+template <typename T>
+static gp_status pack(const OpCtx& c, const T* vals) {
+  int64_t n = c.g->n;
+  unsigned grid = (unsigned)((n + 255) / 256);
+  pack_kernel<T><<<grid, 256, 0, c.st>>>((const T*)c.g->x, vals, (Rec<T>*)c.rec(), n, c.g->d);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+__global__ void finalize_logdet_kernel(const Control* ctrl, double* logdet, double* grad) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    logdet[0] = ctrl->acc[0];
+    if (grad) { grad[0] = ctrl->acc[1]; grad[1] = ctrl->acc[2]; }
+  }
+}
+
+template <typename T>
+static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
+  bool spec = use_spec(c);
+  GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
+  if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr));
+  GP_OK_OR_RETURN(head_factor(c, nullptr, 0));
+  GP_OK_OR_RETURN(head_forward(c, xi, v, c.rec(), spec));
+  const int64_t* off = c.g->batch_off;
+  for (int b = 0; b < c.g->n_batches; ++b)
+    GP_OK_OR_RETURN((launch_range<T, OPK_FORWARD>(c, spec, v, xi, v, off[b], off[b + 1])));
+  return GP_OK;
+}
+
+template <typename T>
+static gp_status inverse_t(const OpCtx& c, const T* v, T* xi) {
+  bool spec = use_spec(c);
+  GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
+  if (spec) GP_OK_OR_RETURN(pack<T>(c, v));
+  GP_OK_OR_RETURN(head_factor(c, v, 1));
+  GP_OK_OR_RETURN(head_inverse_out(c, xi));
+  return launch_range<T, OPK_INVERSE>(c, spec, v, v, xi, c.g->n0, c.g->n);
+}
+
+template <typename T>
+static gp_status logdet_t(const OpCtx& c, double* logdet, double* grad) {
+  bool spec = use_spec(c);
+  GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
+  if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr));
+  GP_OK_OR_RETURN(head_factor(c, nullptr, 0));
+  GP_OK_OR_RETURN(head_logdet(c, &c.ctrl()->acc[0], nullptr));
+  GP_OK_OR_RETURN((launch_range<T, OPK_LOGDET>(c, spec, nullptr, nullptr, nullptr, c.g->n0, c.g->n)));
+  finalize_logdet_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), logdet, grad);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+gp_status run_forward(const OpCtx& c, const void* xi, void* v) {
+  return c.g->dtype == GP_F64 ? forward_t<double>(c, (const double*)xi, (double*)v)
+                              : forward_t<float>(c, (const float*)xi, (float*)v);
+}
+gp_status run_inverse(const OpCtx& c, const void* v, void* xi) {
+  return c.g->dtype == GP_F64 ? inverse_t<double>(c, (const double*)v, (double*)xi)
+                              : inverse_t<float>(c, (const float*)v, (float*)xi);
+}
+gp_status run_logdet(const OpCtx& c, double* logdet, double* grad) {
+  return c.g->dtype == GP_F64 ? logdet_t<double>(c, logdet, grad) : logdet_t<float>(c, logdet, grad);
+}
+
+}  // namespace gp
