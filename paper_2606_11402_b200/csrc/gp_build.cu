@@ -158,9 +158,10 @@ __device__ __forceinline__ double d2_canon(const double* xi, const T* __restrict
 
 template <typename T, int KMAX>
 __global__ void __launch_bounds__(128)
-knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int32_t* __restrict__ nbr) {
+knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int64_t n_threads,
+           int32_t* __restrict__ nbr) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= n) return;
+  if (t >= n_threads) return;
   // thread t -> level l, heap position q -> bit-reversed position p -> tree index i: the queries of one
   // warp are consecutive leaves of the same level, i.e. spatial neighbours
   int l = 63 - __clzll((unsigned long long)(t + 1));
@@ -222,8 +223,15 @@ knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int32_t
 }
 
 // ---- b3: depth ----------------------------------------------------------------------------------------
+__global__ void max_depth_kernel(const int32_t* __restrict__ depth, int64_t n, unsigned long long* out) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  int32_t v = i < n ? depth[i] : 0;
+  for (int o = 16; o > 0; o >>= 1) { int32_t w = __shfl_xor_sync(0xffffffffu, v, o); v = w > v ? w : v; }
+  if ((threadIdx.x & 31) == 0 && v > 0) atomicMax(out, (unsigned long long)v);
+}
+
 __global__ void depth_sweep_kernel(const int32_t* __restrict__ nbr, int64_t n, int64_t n0, int k,
-                                   int32_t* depth, unsigned int* changed) {
+                                   int32_t* depth, unsigned long long* changed) {
   int64_t i = n0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int32_t* row = nbr + (i - n0) * k;
@@ -233,7 +241,7 @@ __global__ void depth_sweep_kernel(const int32_t* __restrict__ nbr, int64_t n, i
     m = dj > m ? dj : m;
   }
   int32_t nd = m + 1;
-  if (((volatile int32_t*)depth)[i] != nd) { ((volatile int32_t*)depth)[i] = nd; *changed = 1u; }
+  if (((volatile int32_t*)depth)[i] != nd) { ((volatile int32_t*)depth)[i] = nd; *changed = 1ULL; }
 }
 
 // ---- b4: depth sort -----------------------------------------------------------------------------------
@@ -312,3 +320,220 @@ __global__ void emit_graph_kernel(const uint32_t* __restrict__ pos2tree, const u
 }
 
 }  // namespace gp
+
+// ---- host driver ----------------------------------------------------------------------------------------
+namespace gp {
+
+static inline unsigned nblk(int64_t n, int t = 256) { return (unsigned)((n + t - 1) / t); }
+
+template <typename KeyT>
+static gp_status sort_pairs(void* tmp, size_t tmp_bytes, cub::DoubleBuffer<KeyT>& keys,
+                            cub::DoubleBuffer<uint32_t>& vals, int64_t m, int begin_bit, int end_bit, cudaStream_t st) {
+  if (m <= 0) return GP_OK;
+  size_t need = 0;
+  GP_CUDA_OK(cub::DeviceRadixSort::SortPairs(nullptr, need, keys, vals, (int)m, begin_bit, end_bit, st));
+  if (need > tmp_bytes) return GP_ERR_WORKSPACE;
+  GP_CUDA_OK(cub::DeviceRadixSort::SortPairs(tmp, need, keys, vals, (int)m, begin_bit, end_bit, st));
+  count_launch(3);
+  return GP_OK;
+}
+
+struct EventSet {
+  cudaEvent_t ev[5];
+  bool ok = true;
+  EventSet() { for (auto& e : ev) if (cudaEventCreate(&e) != cudaSuccess) ok = false; }
+  ~EventSet() { for (auto& e : ev) cudaEventDestroy(e); }
+};
+
+template <typename T>
+static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, int dtype, int flags, int64_t* perm,
+                         T* x_graph, int32_t* nbr, int32_t* depth, int64_t* boff_host, int max_batches,
+                         int32_t* n_batches, char* ws, cudaStream_t st) {
+  BuildLayout L = build_layout(n, d, k, dtype);
+  Control* ctrl = (Control*)(ws + L.ctrl);
+  uint32_t* rank = (uint32_t*)(ws + L.rank);
+  uint64_t* keys_a = (uint64_t*)(ws + L.keys_a);
+  uint64_t* keys_b = (uint64_t*)(ws + L.keys_b);
+  uint32_t* vals_a = (uint32_t*)(ws + L.vals_a);
+  uint32_t* vals_b = (uint32_t*)(ws + L.vals_b);
+  uint32_t* seg = (uint32_t*)(ws + L.seg);
+  uint32_t* perm_tree = (uint32_t*)(ws + L.perm_tree);
+  T* x_tree = (T*)(ws + L.x_tree);
+  int32_t* nbr_tree = (int32_t*)(ws + L.nbr_tree);
+  int32_t* depth_tree = (int32_t*)(ws + L.depth_tree);
+  uint32_t* tree2pos = (uint32_t*)(ws + L.tree2pos);
+  uint32_t* pos2tree = (uint32_t*)(ws + L.pos2tree);
+  unsigned long long* bbox = (unsigned long long*)(ws + L.bbox);
+  int64_t* boff_dev = (int64_t*)(ws + L.boff);
+  void* tmp = ws + L.cub_tmp;
+
+  EventSet E;
+  if (!E.ok) return GP_ERR_CUDA;
+  GP_CUDA_OK(cudaMemsetAsync(ctrl, 0, kCtrlBytes, st));
+  GP_CUDA_OK(cudaEventRecord(E.ev[0], st));
+
+  // ---- b1: order -------------------------------------------------------------------------------------
+  using CoordKey = typename std::conditional<sizeof(T) == 4, uint32_t, uint64_t>::type;
+  for (int dim = 0; dim < d; ++dim) {
+    CoordKey* ck_a = (CoordKey*)keys_a;
+    CoordKey* ck_b = (CoordKey*)keys_b;
+    coord_keys_kernel<T, CoordKey><<<nblk(n), 256, 0, st>>>(x_user, n, d, dim, ck_a, vals_a);
+    GP_LAUNCH_CHECK();
+    cub::DoubleBuffer<CoordKey> kb(ck_a, ck_b);
+    cub::DoubleBuffer<uint32_t> vb(vals_a, vals_b);
+    GP_OK_OR_RETURN(sort_pairs<CoordKey>(tmp, L.cub_bytes, kb, vb, n, 0, (int)sizeof(CoordKey) * 8, st));
+    scatter_rank_kernel<<<nblk(n), 256, 0, st>>>(vb.Current(), n, rank + (size_t)dim * n);
+    GP_LAUNCH_CHECK();
+  }
+  const TreeShape shape = tree_shape(n);
+  int rank_bits = 1;
+  while (((int64_t)1 << rank_bits) < n) ++rank_bits;
+  {
+    cub::DoubleBuffer<uint64_t> kb(keys_a, keys_b);
+    cub::DoubleBuffer<uint32_t> vb(vals_a, vals_b);
+    iota_seg_kernel<<<nblk(n), 256, 0, st>>>(vb.Current(), seg, n);
+    GP_LAUNCH_CHECK();
+    int64_t m_sort = n;
+    for (int l = 0; l <= shape.lam; ++l) {
+      // elements retired at level l-1 carry segment id 2^l and sink behind the active ones in this sort
+      level_keys_kernel<<<nblk(m_sort), 256, 0, st>>>(vb.Current(), seg, rank + (size_t)(l % d) * n, m_sort,
+                                                      rank_bits, kb.Current());
+      GP_LAUNCH_CHECK();
+      GP_OK_OR_RETURN(sort_pairs<uint64_t>(tmp, L.cub_bytes, kb, vb, m_sort, 0, rank_bits + l + 1, st));
+      int64_t m_active = l == 0 ? n : m_sort - ((int64_t)1 << (l - 1));
+      level_split_kernel<<<nblk(m_active), 256, 0, st>>>(kb.Current(), vb.Current(), m_active, rank_bits, l, shape,
+                                                         seg, perm_tree);
+      GP_LAUNCH_CHECK();
+      m_sort = m_active;
+    }
+  }
+  gather_points_kernel<T><<<nblk(n), 256, 0, st>>>(x_user, perm_tree, n, d, x_tree);
+  GP_LAUNCH_CHECK();
+  GP_CUDA_OK(cudaEventRecord(E.ev[1], st));
+
+  // ---- b2: preceding kNN -----------------------------------------------------------------------------
+  if (n > n0) {
+    int64_t n_threads = ((int64_t)2 << shape.lam) - 1;
+    if (k <= 16) knn_kernel<T, 16><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree);
+    else if (k <= 32) knn_kernel<T, 32><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree);
+    else knn_kernel<T, 64><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree);
+    GP_LAUNCH_CHECK();
+  }
+  GP_CUDA_OK(cudaEventRecord(E.ev[2], st));
+
+  // ---- b3: depth fixed point --------------------------------------------------------------
+  GP_CUDA_OK(cudaMemsetAsync(depth_tree, 0, (size_t)n * 4, st));
+  int64_t max_depth = 0;
+  if (n > n0) {
+    unsigned long long* flag = &ctrl->pad0;
+    for (int guard = 0; guard < (1 << 22); ++guard) {
+      for (int r = 0; r < 3; ++r) {
+        depth_sweep_kernel<<<nblk(n - n0), 256, 0, st>>>(nbr_tree, n, n0, k, depth_tree, flag);
+        GP_LAUNCH_CHECK();
+      }
+      GP_CUDA_OK(cudaMemsetAsync(flag, 0, 8, st));
+      depth_sweep_kernel<<<nblk(n - n0), 256, 0, st>>>(nbr_tree, n, n0, k, depth_tree, flag);
+      GP_LAUNCH_CHECK();
+      unsigned long long h = 0;
+      GP_CUDA_OK(cudaMemcpyAsync(&h, flag, 8, cudaMemcpyDeviceToHost, st));
+      GP_CUDA_OK(cudaStreamSynchronize(st));
+      if (!h) break;
+    }
+    unsigned long long* mx = &ctrl->ticket;
+    max_depth_kernel<<<nblk(n), 256, 0, st>>>(depth_tree, n, mx);
+    GP_LAUNCH_CHECK();
+    unsigned long long h = 0;
+    GP_CUDA_OK(cudaMemcpyAsync(&h, mx, 8, cudaMemcpyDeviceToHost, st));
+    GP_CUDA_OK(cudaStreamSynchronize(st));
+    max_depth = (int64_t)h;
+    if (max_depth > max_batches || max_depth > kMaxBatches) return GP_ERR_INVALID_ARG;
+  }
+  GP_CUDA_OK(cudaEventRecord(E.ev[3], st));
+
+  // ---- b4: depth sort, remap ---------------------------------------------------------------------------
+  if (n > n0) {
+    int depth_bits = 1;
+    while (((int64_t)1 << depth_bits) <= max_depth) ++depth_bits;
+    const int spatial = (flags & GP_BUILD_SPATIAL_BATCHES) ? 1 : 0;
+    int cell_bits = 0, depth_shift = 0;
+    if (spatial) {
+      cell_bits = (63 - depth_bits) / d;
+      if (cell_bits > 21) cell_bits = 21;
+      depth_shift = cell_bits * d;
+      GP_CUDA_OK(cudaMemsetAsync(bbox, 0xff, 8 * 2 * kMaxD, st));
+      for (int t = 0; t < d; ++t) GP_CUDA_OK(cudaMemsetAsync(bbox + 2 * t + 1, 0, 8, st));
+      bbox_kernel<T><<<nblk(n), 256, 0, st>>>(x_tree, n, d, bbox);
+      GP_LAUNCH_CHECK();
+    }
+    cub::DoubleBuffer<uint64_t> kb(keys_a, keys_b);
+    cub::DoubleBuffer<uint32_t> vb(vals_a, vals_b);
+    sort_keys_kernel<T><<<nblk(n - n0), 256, 0, st>>>(x_tree, depth_tree, n, n0, d, spatial, cell_bits, depth_shift,
+                                                      bbox, kb.Current(), vb.Current());
+    GP_LAUNCH_CHECK();
+    GP_OK_OR_RETURN(sort_pairs<uint64_t>(tmp, L.cub_bytes, kb, vb, n - n0, 0, depth_shift + depth_bits, st));
+    positions_kernel<<<nblk(n), 256, 0, st>>>(vb.Current(), n, n0, pos2tree, tree2pos);
+    GP_LAUNCH_CHECK();
+  } else {
+    positions_kernel<<<nblk(n), 256, 0, st>>>(nullptr, n, n0, pos2tree, tree2pos);
+    GP_LAUNCH_CHECK();
+  }
+  emit_graph_kernel<T><<<nblk(n), 256, 0, st>>>(pos2tree, tree2pos, perm_tree, x_tree, depth_tree, nbr_tree, n, n0, d, k,
+                                                perm, x_graph, depth, nbr, boff_dev);
+  GP_LAUNCH_CHECK();
+  GP_CUDA_OK(cudaEventRecord(E.ev[4], st));
+  if (max_depth > 0)
+    GP_CUDA_OK(cudaMemcpyAsync(boff_host, boff_dev, (size_t)(max_depth + 1) * 8, cudaMemcpyDeviceToHost, st));
+  GP_CUDA_OK(cudaStreamSynchronize(st));
+  if (max_depth == 0) boff_host[0] = n0;
+  *n_batches = (int32_t)max_depth;
+  Control h{};
+  for (int s = 0; s < 4; ++s) {
+    float ms = 0.f;
+    GP_CUDA_OK(cudaEventElapsedTime(&ms, E.ev[s], E.ev[s + 1]));
+    h.build_ms[s] = ms;
+  }
+  GP_CUDA_OK(cudaMemcpy(ctrl->build_ms, h.build_ms, sizeof(h.build_ms), cudaMemcpyHostToDevice));
+  return GP_OK;
+}
+}  // namespace gp
+
+using namespace gp;
+
+extern "C" {
+
+size_t gp_graph_build_workspace_bytes(int64_t n, int32_t d, int32_t k, int32_t dtype) {
+  if (n <= 0 || d < 1 || d > kMaxD || k < 1 || k > kMaxK || (dtype != GP_F32 && dtype != GP_F64)) return 0;
+  return build_layout(n, d, k, dtype).total;
+}
+
+gp_status gp_graph_build(const void* x_user, int64_t n, int32_t d, int32_t k, int64_t n0, int32_t dtype,
+                         int32_t build_flags, int64_t* perm, void* x_graph, int32_t* nbr, int32_t* depth,
+                         int64_t* batch_off_host, int32_t max_batches, int32_t* n_batches, void* ws, size_t ws_bytes,
+                         void* cuda_stream) {
+  if (!x_user || !perm || !x_graph || !depth || !batch_off_host || !n_batches) return GP_ERR_INVALID_ARG;
+  if (n <= 0 || n0 < 0 || n0 > n || d < 1 || k < 1 || max_batches < 1) return GP_ERR_INVALID_ARG;
+  if (d > kMaxD || k > kMaxK || n >= (1LL << 31)) return GP_ERR_UNSUPPORTED;
+  if (dtype != GP_F32 && dtype != GP_F64) return GP_ERR_INVALID_ARG;
+  if (n0 < k && n0 < n) return GP_ERR_INVALID_ARG;
+  if (n > n0 && !nbr) return GP_ERR_INVALID_ARG;
+  size_t need = gp_graph_build_workspace_bytes(n, d, k, dtype);
+  if (!ws || ws_bytes < need || (((uintptr_t)ws) & 255) != 0) return GP_ERR_WORKSPACE;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return GP_ERR_CUDA;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  if (dtype == GP_F64)
+    return build_t<double>((const double*)x_user, n, d, k, n0, dtype, build_flags, perm, (double*)x_graph, nbr, depth,
+                           batch_off_host, max_batches, n_batches, (char*)ws, st);
+  return build_t<float>((const float*)x_user, n, d, k, n0, dtype, build_flags, perm, (float*)x_graph, nbr, depth,
+                        batch_off_host, max_batches, n_batches, (char*)ws, st);
+}
+
+gp_status gp_graph_build_times(void* ws, double* ms4_host) {
+  if (!ws || !ms4_host) return GP_ERR_INVALID_ARG;
+  Control h;
+  GP_CUDA_OK(cudaMemcpy(&h, ws, sizeof(Control), cudaMemcpyDeviceToHost));
+  for (int s = 0; s < 4; ++s) ms4_host[s] = h.build_ms[s];
+  return GP_OK;
+}
+
+}  // extern "C"
