@@ -1,0 +1,415 @@
+"""bench.py — GraphGP Vecchia conditioning path on B200: points/s and fraction of roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl graft|reference] [--config C] [--n N]
+
+A "step" is one pass of the whole hot path over one synthetic workload: gp_forward (dense
+head + every batch), gp_inverse, gp_logdet and gp_vjp, each over all N points of BASELINE.json's headline
+configuration (config 3: N = 2^24 clustered 3-d points, k = 16, Matern-3/2, fp32).  The graph is built once by
+gp_graph_build outside the timed region (timed separately, reported under "builder").  `value` = N / step
+time; per-operation rates and roofline fractions are under "ops".  One JSON line on stdout (rank 0).
+
+Multi-GPU: the forward pass does not shard: `--gpus N` runs N independent replicas (one noise
+vector each on a replicated graph), no data-path collective, scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import gp_workloads as W  # noqa: E402
+
+METRIC = "Vecchia forward/inverse points/sec at N=2^24,k=16 fp32; % of roofline"
+UNIT = "points/s"
+# nominal non-tensor FP32 peak the ALU roofline is taken against: 148 SM x 128 lanes x 2 x 1.965 GHz
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+FP64_PEAK_TFLOPS = FP32_PEAK_TFLOPS / 2
+HBM_FALLBACK_GBS = 6650.0
+
+
+def algorithmic_work(k: int, d: int, kind: str, B: int, op: str):
+    """(flop, bytes) per conditioned point: SURVEY.md §8(d) closed forms."""
+    n = k + 1
+    P = k * (k + 1) // 2
+    fma = (n - 1) * n * (n + 1) // 6 + k * (k - 1) // 2 + k + 1
+    mul = n * (n - 1) // 2 + k
+    fk = {"se": 3, "matern32": 6, "exp": 3}[kind]
+    flop = 2 * fma + mul + P * (3 * d - 1) + P * fk + n
+    if op == "logdet":
+        byt = 4 * k + (k + 1) * d * B
+    else:
+        byt = 4 * k + k * (d + 1) * B + d * B + 2 * B
+    if op == "vjp":
+        # second triangle sweep for K_bar (back-substitutions for w and alpha, pair derivative, accumulation)
+        flop += 2 * (k * (k + 1)) + P * (fk + 6) + 4 * k
+        byt += 4 * B + 2 * 4 * k
+    return flop, byt
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured"
+    return HBM_FALLBACK_GBS, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, dev: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-i", str(dev), "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            c = [t.strip() for t in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])); mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, c[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def setup_dist(args):
+    import torch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_mod
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", "29511")
+        dist_mod.init_process_group("nccl" if torch.cuda.is_available() else "gloo", rank=rank, world_size=world)
+        dist = dist_mod
+    return dist, world, rank, local
+
+
+def make_workload(cfg, n, dtype, rank):
+    """Seeded synthetic inputs: points in user order, xi and v_bar per replica."""
+    x = W.make_points(cfg, dtype, n)
+    xi = W.make_noise(cfg.cid + 100 * rank, n, dtype, "xi")
+    vbar = W.make_noise(cfg.cid + 100 * rank, n, dtype, "vbar")
+    return x, xi, vbar
+
+
+def oracle_sample(cfg, G, xi_h, vbar_h, v_gpu_h, target_s=15.0):
+    """Oracle (as it stands, fp64, OpenMP over the points of a batch) on a PREFIX of the same graph: the first
+    M graph positions are themselves a valid generation graph (every neighbour precedes its point)."""
+    import oracle as orc
+    orc.build()
+    OK = orc.Kernel(cfg.kind, cfg.sigma, cfg.ell, cfg.jitter)
+    n, n0, k = G.n, G.n0, G.k
+
+    def run(M):
+        xg = G.x[:M].cpu().numpy().astype(np.float64)
+        nbr = G.nbr[:M - n0].cpu().numpy()
+        boff = np.unique(np.minimum(G.batch_off, M))
+        xi64 = xi_h[:M].astype(np.float64)
+        t0 = time.perf_counter()
+        v = orc.forward(xg, OK, xi64, n0=n0, k=k, nbr=nbr, batch_off=boff)
+        t1 = time.perf_counter()
+        orc.inverse(xg, OK, v, n0=n0, k=k, nbr=nbr)
+        t2 = time.perf_counter()
+        orc.logdet(xg, OK, n0=n0, k=k, nbr=nbr)
+        t3 = time.perf_counter()
+        orc.vjp(xg, OK, xi64, v, vbar_h[:M].astype(np.float64), n0=n0, k=k, nbr=nbr, batch_off=boff)
+        t4 = time.perf_counter()
+        return v, dict(forward=t1 - t0, inverse=t2 - t1, logdet=t3 - t2, vjp=t4 - t3)
+
+    # calibrate on growing prefixes (the dense head and thread start-up dominate small ones), then one run sized
+    # for about target_s seconds of CPU work
+    M = min(n, max(4 * n0, 1 << 16))
+    v, t = run(M)
+    tot = sum(t.values())
+    for _ in range(3):
+        M2 = int(min(n, M * target_s / max(tot, 1e-3)))
+        if M2 < 2 * M:
+            break
+        M = min(n, 1 << int(np.floor(np.log2(M2))))
+        v, t = run(M)
+        tot = sum(t.values())
+    err = None
+    if v_gpu_h is not None:
+        err = float(np.abs(v_gpu_h[:M].astype(np.float64) - v).max() / v.std())
+    return dict(M=M, seconds=t, total_s=tot, cores=orc.num_threads(), v_err_over_std=err)
+
+
+def run_graft(args):
+    import torch
+    import paper_2606_11402_b200 as gp
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    dist, world, rank, local = setup_dist(args)
+    if world != args.gpus and rank == 0:
+        print(f"# note: --gpus {args.gpus} but WORLD_SIZE={world}; using WORLD_SIZE", file=sys.stderr)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    gp.lib()
+    cfg = W.CONFIGS[args.config]
+    n = args.n or cfg.n
+    dtype = args.dtype or cfg.dtypes[0]
+    B = 8 if dtype == "f64" else 4
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    K = gp.Kernel(cfg.kind, cfg.sigma, cfg.ell, cfg.jitter)
+
+    x_h, xi_h, vbar_h = make_workload(cfg, n, dtype, rank)
+    x_user = torch.as_tensor(x_h, device=dev)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    G = gp.gp_graph_build(x_user, cfg.k, cfg.n0)
+    torch.cuda.synchronize()
+    build_wall = time.perf_counter() - t0
+    del x_user
+    L = len(G.batch_off) - 1
+    xi = torch.as_tensor(xi_h, device=dev)
+    vbar = torch.as_tensor(vbar_h, device=dev)
+    v = torch.empty_like(xi)
+    xi_back = torch.empty_like(xi)
+    st = torch.cuda.current_stream()
+
+    ops = ["forward", "inverse", "logdet", "vjp"]
+    state = {}
+
+    def do(op):
+        if op == "forward":
+            gp.gp_forward(G, K, xi, out=v)
+        elif op == "inverse":
+            gp.gp_inverse(G, K, v, out=xi_back)
+        elif op == "logdet":
+            state["logdet"] = gp.gp_logdet(G, K)
+        else:
+            state["xi_bar"], state["theta_bar"] = gp.gp_vjp(G, K, xi, v, vbar)
+
+    for _ in range(max(args.warmup, 0)):
+        for op in ops:
+            do(op)
+    torch.cuda.synchronize()
+    for op in ("forward", "inverse", "logdet", "vjp"):
+        nbad = gp.check_errors(G.workspace({"forward": gp.GP_OP_FORWARD, "inverse": gp.GP_OP_INVERSE,
+                                            "logdet": gp.GP_OP_LOGDET, "vjp": gp.GP_OP_VJP}[op]))
+        if nbad:
+            raise RuntimeError(f"{op}: {nbad} points were not positive definite")
+
+    # ---- device-resident timing ---------------------------------------------------------------------
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(len(ops) + 1)] for _ in range(args.steps)]
+    if dist:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local) if rank == 0 else None
+    launches0 = gp.launch_count()
+    for s in range(args.steps):
+        ev[s][0].record(st)
+        for j, op in enumerate(ops):
+            do(op)
+            ev[s][j + 1].record(st)
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    launches = gp.launch_count() - launches0
+    clocks = sampler.stop() if sampler else None
+    total_ms = sum(ev[s][0].elapsed_time(ev[s][len(ops)]) for s in range(args.steps))
+    op_ms = {op: float(np.mean([ev[s][j].elapsed_time(ev[s][j + 1]) for s in range(args.steps)]))
+             for j, op in enumerate(ops)}
+    if dist:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * n / (ms_per_step * 1e-3)
+    v_gpu_h = v.cpu().numpy() if rank == 0 else None
+
+    # ---- end to end: host (pinned) buffers through the C ABI's *_host calls ------------------------------
+    xi_p = torch.as_tensor(xi_h).pin_memory()
+    vbar_p = torch.as_tensor(vbar_h).pin_memory()
+    v_p = torch.empty_like(xi_p).pin_memory()
+    xi2_p = torch.empty_like(xi_p).pin_memory()
+    xib_p = torch.empty_like(xi_p).pin_memory()
+    in_dev, out_dev = torch.empty_like(xi), torch.empty_like(xi)
+    tb_p = torch.empty(2, dtype=torch.float64).pin_memory()
+    ld_p = torch.empty(1, dtype=torch.float64).pin_memory()
+    staging = (in_dev, out_dev, torch.empty_like(xi), torch.empty_like(xi), torch.empty(2, dtype=torch.float64, device=dev))
+
+    def e2e_step():
+        gp.gp_forward_host(G, K, xi_p, v_p, in_dev, out_dev)
+        gp.gp_inverse_host(G, K, v_p, xi2_p, in_dev, out_dev)
+        ld_p.copy_(gp.gp_logdet(G, K), non_blocking=True)
+        gp.gp_vjp_host(G, K, xi_p, v_p, vbar_p, xib_p, tb_p, staging)
+
+    e2e_step()
+    torch.cuda.synchronize()
+    if dist:
+        dist.barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(st)
+    for _ in range(args.steps):
+        e2e_step()
+    e1.record(st)
+    torch.cuda.synchronize()
+    e2e_ms = e0.elapsed_time(e1) / args.steps
+    if dist:
+        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    h2d = n * B * (1 + 1 + 3)          # forward xi; inverse v; vjp xi, v, v_bar
+    d2h = n * B * 3 + 8 + 16           # v; xi; xi_bar; logdet; theta_bar
+
+    if rank != 0:
+        return
+    hbm, peak_src = measured_peaks()
+    alu_peak = FP64_PEAK_TFLOPS if dtype == "f64" else FP32_PEAK_TFLOPS
+    npts = n - G.n0
+    ops_out = {}
+    for op in ops:
+        flop, byt = algorithmic_work(cfg.k, cfg.d, cfg.kind, B, op)
+        t_s = op_ms[op] * 1e-3
+        t_alu, t_hbm = flop * npts / (alu_peak * 1e12), byt * npts / (hbm * 1e9)
+        ops_out[op] = dict(ms=round(op_ms[op], 4), points_per_s=n / t_s, flop_per_point=flop, bytes_per_point=byt,
+                           tflops=flop * npts / t_s / 1e12, gbs=byt * npts / t_s / 1e9,
+                           roofline_frac=max(t_alu, t_hbm) / t_s, bound="alu" if t_alu >= t_hbm else "hbm")
+    f = ops_out["forward"]
+    flop, byt = algorithmic_work(cfg.k, cfg.d, cfg.kind, B, "forward")
+    if f["bound"] == "alu":
+        roof = dict(bound="alu", achieved=f["tflops"], peak=alu_peak, unit="TFLOP/s", frac=f["tflops"] / alu_peak,
+                    traffic=None, peak_source="nominal non-tensor peak, 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz",
+                    hbm_frac=f["gbs"] / hbm, hbm_peak_source=peak_src)
+    else:
+        roof = dict(bound="hbm", achieved=f["gbs"], peak=hbm, unit="GB/s", frac=f["gbs"] / hbm, traffic=None,
+                    peak_source=peak_src)
+    roof["kernel"] = "gp_forward (dense head + all batches), CUDA events on the launching stream"
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": dtype, "data": "synthetic",
+        "config": {"workload": f"config {cfg.cid}: {cfg.name}, N={n}, d={cfg.d}, k={cfg.k}, n0={cfg.n0}, "
+                               f"{cfg.kind} sigma={cfg.sigma} ell={cfg.ell} jitter={cfg.jitter}",
+                   "step": "gp_forward + gp_inverse + gp_logdet + gp_vjp, each over all N points",
+                   "n_batches": L, "parallelism": "replicas" if world > 1 else "single GPU",
+                   "l2": "inputs larger than L2 (nbr %.0f MiB + records %.0f MiB per op)" % (
+                       npts * cfg.k * 4 / 2 ** 20, n * 4 * B / 2 ** 20)},
+        "ops": ops_out, "roofline": roof,
+        "e2e": {"value": world * n / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+        "gpu_launches": int(launches), "clocks": clocks,
+        "builder": {"wall_s": build_wall, "stage_ms": {k_: float(v_) for k_, v_ in
+                                                       zip(("order", "knn", "depth", "sort"), G.build_ms)}},
+    }
+    if not args.no_cpu_baseline:
+        smp = oracle_sample(cfg, G, xi_h, vbar_h, v_gpu_h, target_s=args.cpu_seconds)
+        out["cpu_baseline"] = {"value": smp["M"] / smp["total_s"], "unit": UNIT, "cores": smp["cores"], "kind": "oracle",
+                               "sample": f"first {smp['M']} graph positions of the same graph "
+                                         f"(forward+inverse+logdet+vjp, fp64, {smp['total_s']:.1f} s)",
+                               "seconds": smp["seconds"]}
+        out["parity_on_sample"] = {"max_abs_dv_over_std": smp["v_err_over_std"], "points": smp["M"]}
+    print(json.dumps(out))
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores (this tier has no other reference).  Each
+    step is a bounded sample of the same workload: a prefix of the generation graph.  The graph itself comes from
+    the oracle's own builder when the sample is small enough for its O(N^2) neighbour search, which bounds the
+    sample; nothing of the CUDA path runs in this arm."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as orc
+    orc.build()
+    cfg = W.CONFIGS[args.config]
+    dtype = args.dtype or cfg.dtypes[0]
+    M = args.n or args.reference_points
+    x = W.make_points(cfg, dtype, M).astype(np.float64)
+    g = orc.build_graph(x, cfg.k, min(cfg.n0, M))
+    OK = orc.Kernel(cfg.kind, cfg.sigma, cfg.ell, cfg.jitter)
+    xi = W.make_noise(cfg.cid, M, dtype, "xi").astype(np.float64)
+    vbar = W.make_noise(cfg.cid, M, dtype, "vbar").astype(np.float64)
+
+    def step():
+        v = orc.forward(g.x, OK, xi, n0=g.n0, k=g.k, nbr=g.nbr, batch_off=g.batch_off)
+        orc.inverse(g.x, OK, v, n0=g.n0, k=g.k, nbr=g.nbr)
+        orc.logdet(g.x, OK, n0=g.n0, k=g.k, nbr=g.nbr)
+        orc.vjp(g.x, OK, xi, v, vbar, n0=g.n0, k=g.k, nbr=g.nbr, batch_off=g.batch_off)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / args.steps
+    value = M / dt
+    sample = (f"{M} points drawn by config {cfg.cid}'s recipe (the first {M} user points), graph by the oracle's own "
+              f"order + brute-force neighbours; forward+inverse+logdet+vjp in fp64")
+    out = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", 1)),
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"config {cfg.cid}: {cfg.name}, bounded sample of {M} points, d={cfg.d}, k={cfg.k}, "
+                               f"n0={min(cfg.n0, M)}, {cfg.kind} ell={cfg.ell} jitter={cfg.jitter}",
+                   "step": "forward + inverse + logdet + vjp over the sample"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="graft", choices=["graft", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configuration (1-5); 3 = the headline")
+    ap.add_argument("--n", type=int, default=0, help="override the number of points (smaller dry runs)")
+    ap.add_argument("--dtype", default="", choices=["", "f32", "f64"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")
+    ap.add_argument("--reference-points", type=int, default=1 << 16)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_graft(args)
+
+
+if __name__ == "__main__":
+    main()

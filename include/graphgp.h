@@ -109,6 +109,14 @@ gp_status gp_forward_host(const gp_graph* g, const gp_kernel* kern, const void* 
 gp_status gp_inverse_host(const gp_graph* g, const gp_kernel* kern, const void* v_host, void* xi_host,
                           void* in_dev, void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream);
 
+/* gp_vjp with HOST xi, v, v_bar (in) and xi_bar, theta_bar[2] (out): three [n] host->device copies into the
+ * device staging buffers xi_dev, v_dev, v_bar_dev, the VJP, then xi_bar_dev -> xi_bar_host and theta_bar_dev ->
+ * theta_bar_host, all on `cuda_stream`.  The caller synchronises the stream before reading the results.  */
+gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_host, const void* v_host,
+                      const void* v_bar_host, void* xi_bar_host, double* theta_bar_host, void* xi_dev, void* v_dev,
+                      void* v_bar_dev, void* xi_bar_dev, double* theta_bar_dev, void* ws, size_t ws_bytes,
+                      void* cuda_stream);
+
 /* Graph construction, separately timed, "plain":
  *   order   bit-reversed left-balanced k-d tree: node i at level l has children i+2^l, i+2^(l+1);
  *           split dimension = level mod d; ties by (coordinate, user id)             (R-3, R-4)

@@ -24,7 +24,7 @@ GP_BUILD_SPATIAL_BATCHES = 1
 KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
 
 EXPORTS = ["gp_workspace_bytes", "gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host",
-           "gp_inverse_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
+           "gp_inverse_host", "gp_vjp_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
            "gp_check_errors", "gp_status_string", "gp_has_specialised", "gp_launch_count"]
 
 
@@ -72,12 +72,13 @@ def lib():
         L.gp_vjp.argtypes = gk + [vp, vp, vp, vp, vp, vp, sz, vp]
         L.gp_forward_host.argtypes = gk + [vp, vp, vp, vp, vp, sz, vp]
         L.gp_inverse_host.argtypes = gk + [vp, vp, vp, vp, vp, sz, vp]
+        L.gp_vjp_host.argtypes = gk + [vp] * 11 + [sz, vp]
         L.gp_graph_build.argtypes = [vp, C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32, C.c_int32, vp, vp,
                                      vp, vp, vp, C.c_int32, C.POINTER(C.c_int32), vp, sz, vp]
         L.gp_graph_build_times.argtypes = [vp, vp]
         L.gp_check_errors.argtypes = [vp, C.POINTER(C.c_int64)]
         for name in ("gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host", "gp_inverse_host",
-                     "gp_graph_build", "gp_graph_build_times", "gp_check_errors"):
+                     "gp_vjp_host", "gp_graph_build", "gp_graph_build_times", "gp_check_errors"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -258,6 +259,20 @@ def gp_inverse_host(graph: Graph, kern: Kernel, v_host, xi_host, in_dev, out_dev
                                  out_dev.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
            "gp_inverse_host")
     return xi_host
+
+
+def gp_vjp_host(graph: Graph, kern: Kernel, xi_host, v_host, vbar_host, xibar_host, theta_bar_host, staging,
+                stream=None):
+    """End-to-end VJP with HOST (pinned) xi, v, v_bar -> xi_bar, theta_bar.  staging = (xi_dev, v_dev, v_bar_dev,
+    xi_bar_dev, theta_bar_dev): caller-owned device buffers.  Synchronise the stream before reading the results."""
+    ws = graph.workspace(GP_OP_VJP)
+    g, k = graph.c(), kern.c()
+    xd, vd, vbd, xbd, tbd = staging
+    _check(lib().gp_vjp_host(C.byref(g), C.byref(k), xi_host.data_ptr(), v_host.data_ptr(), vbar_host.data_ptr(),
+                             xibar_host.data_ptr(), theta_bar_host.data_ptr(), xd.data_ptr(), vd.data_ptr(),
+                             vbd.data_ptr(), xbd.data_ptr(), tbd.data_ptr(), ws.data_ptr(), ws.numel(),
+                             _stream_ptr(stream)), "gp_vjp_host")
+    return xibar_host, theta_bar_host
 
 
 def gp_graph_build(x_user, k: int, n0: int, build_flags: int = GP_BUILD_SPATIAL_BATCHES, max_batches: int = 1 << 16,

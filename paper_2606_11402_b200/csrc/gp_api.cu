@@ -108,6 +108,24 @@ gp_status gp_inverse_host(const gp_graph* g, const gp_kernel* kern, const void* 
   return GP_OK;
 }
 
+gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_host, const void* v_host,
+                      const void* v_bar_host, void* xi_bar_host, double* theta_bar_host, void* xi_dev, void* v_dev,
+                      void* v_bar_dev, void* xi_bar_dev, double* theta_bar_dev, void* ws, size_t ws_bytes,
+                      void* cuda_stream) {
+  if (!g || !xi_host || !v_host || !v_bar_host || !xi_bar_host || !theta_bar_host || !xi_dev || !v_dev || !v_bar_dev ||
+      !xi_bar_dev || !theta_bar_dev)
+    return GP_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  size_t bytes = (size_t)g->n * dtype_bytes(g->dtype);
+  GP_CUDA_OK(cudaMemcpyAsync(xi_dev, xi_host, bytes, cudaMemcpyHostToDevice, st));
+  GP_CUDA_OK(cudaMemcpyAsync(v_dev, v_host, bytes, cudaMemcpyHostToDevice, st));
+  GP_CUDA_OK(cudaMemcpyAsync(v_bar_dev, v_bar_host, bytes, cudaMemcpyHostToDevice, st));
+  GP_OK_OR_RETURN(gp_vjp(g, kern, xi_dev, v_dev, v_bar_dev, xi_bar_dev, theta_bar_dev, ws, ws_bytes, cuda_stream));
+  GP_CUDA_OK(cudaMemcpyAsync(xi_bar_host, xi_bar_dev, bytes, cudaMemcpyDeviceToHost, st));
+  GP_CUDA_OK(cudaMemcpyAsync(theta_bar_host, theta_bar_dev, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  return GP_OK;
+}
+
 gp_status gp_check_errors(void* ws, int64_t* n_bad_points) {
   if (!ws || !n_bad_points) return GP_ERR_INVALID_ARG;
   Control h;

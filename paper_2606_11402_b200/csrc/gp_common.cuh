@@ -165,7 +165,7 @@ inline size_t dtype_bytes(int dtype) { return dtype == GP_F64 ? 8 : 4; }
 // Workspace layout (byte offsets from ws).  The head is always factored in fp64.
 //   ctrl     Control
 //   boff     device copy of batch_off (int64 [n_batches + 1]) + chunk prefix (int64 [n_batches + 1])
-//   head     (n0 + carried) x n0 doubles: factor of K_head/sigma^2 + carried rows
+//   head     (n0 + carried) x n0 doubles: factor of K_head/sigma^2 + carried rows (+ n0 doubles for the VJP)
 //   rec      packed records Rec<T>[n]                          (register-resident kernels only)
 //   g        VJP: running cotangent, T[n]
 struct WsLayout {
@@ -179,10 +179,11 @@ inline WsLayout ws_layout(const gp_graph* g, int op) {
   size_t off = 0;
   w.ctrl_off = off; off += kCtrlBytes;
   w.boff_off = off; off += align_up(2 * ((size_t)g->n_batches + 1) * sizeof(int64_t), 256);
-  size_t carried = (op == GP_OP_INVERSE) ? 1 : (op == GP_OP_VJP ? n0 : 0);
+  // carried rows: inverse 1 (v_head); gradients 2 n0 (identity -> L^-T, and ell dM/dell -> its L^-1 image)
+  size_t carried = (op == GP_OP_INVERSE) ? 1 : (op == GP_OP_VJP ? 2 * n0 : 0);
   w.head_rows = n0 + carried;
   size_t head_elems = w.head_rows * n0;
-  if (op == GP_OP_VJP) head_elems += 2 * n0 * n0;  // scratch for L^T Lbar and the K_bar products
+  if (op == GP_OP_VJP) head_elems += n0;  // p = L^T g_head
   w.head_off = off; off += align_up(head_elems * sizeof(double), 256);
   w.rec_off = off; off += align_up(n * 4 * B, 256);
   w.g_off = off;
@@ -209,14 +210,17 @@ struct OpCtx {
 gp_status head_factor(const OpCtx& c, const void* carried_src /*dtype [n0] or null*/, int n_carried);
 gp_status head_forward(const OpCtx& c, const void* xi, void* v, void* rec, bool rec_is_packed);
 gp_status head_inverse_out(const OpCtx& c, void* xi);
-gp_status head_logdet(const OpCtx& c, double* acc /*device: acc[0] += logdet head*/, double* grad_acc);
-gp_status head_vjp(const OpCtx& c, const void* xi, const void* gbar, void* xibar, double* acc);
+gp_status head_logdet(const OpCtx& c, double* acc /*device: acc[0] += logdet head*/,
+                      double* grad_ell_acc /*device or null: += ell * d/dell, needs head_factor(c, nullptr, 2 n0)*/);
+gp_status head_vjp(const OpCtx& c, const void* xi, const void* gbar, void* xibar,
+                   double* acc /*device: acc[0] += sigma_bar, acc[1] += ell * ell_bar*/);
 
 // conditioning (gp_ops.cu, gp_vjp.cu)
 gp_status run_forward(const OpCtx& c, const void* xi, void* v);
 gp_status run_inverse(const OpCtx& c, const void* v, void* xi);
 gp_status run_logdet(const OpCtx& c, double* logdet, double* grad);
 gp_status run_vjp(const OpCtx& c, const void* xi, const void* v, const void* vbar, void* xibar, double* thetabar);
+gp_status run_logdet_grad(const OpCtx& c);   // conditioning part of d logdet / d ell into ctrl->acc[2]
 bool has_specialised(int dtype, int k, int d, int kind);
 
 }  // namespace gp

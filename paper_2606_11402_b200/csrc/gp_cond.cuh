@@ -60,18 +60,20 @@ template <typename T> struct Cond {
   bool ok;
 };
 
-// Register-resident conditioning.  `self` holds the point's own coordinates (its .v is unused here).
-template <typename T, int K, int D, int KIND, bool COHERENT>
-__device__ __forceinline__ Cond<T> condition_reg(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ row,
-                                                 const Rec<T>& self, const KParams<T>& kp) {
-  int32_t idx[K];
+// Register-resident conditioning, in three pieces so that the gradient kernels (gp_vjp.cu) can keep the
+// factor.  Every loop is fully unrolled: no register array is ever indexed dynamically.
+template <typename T, int K, bool COHERENT>
+__device__ __forceinline__ void gather_reg(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ row,
+                                           int32_t (&idx)[K], Rec<T> (&R)[K]) {
   load_row<K>(row, idx);
-  Rec<T> R[K];
 #pragma unroll
   for (int j = 0; j < K; ++j) R[j] = load_rec<COHERENT>(rec + idx[j]);
+}
 
-  // joint matrix, lower triangle, rows 0..K-1 = neighbours, row K = the point itself
-  T A[(K + 1) * (K + 2) / 2];
+// joint matrix M = K / sigma^2, lower triangle, rows 0..K-1 = neighbours, row K = the point itself
+template <typename T, int K, int D, int KIND>
+__device__ __forceinline__ void build_joint_reg(const Rec<T> (&R)[K], const Rec<T>& self, const KParams<T>& kp,
+                                                T (&A)[(K + 1) * (K + 2) / 2]) {
 #pragma unroll
   for (int r = 0; r <= K; ++r) {
 #pragma unroll
@@ -81,11 +83,12 @@ __device__ __forceinline__ Cond<T> condition_reg(const Rec<T>* __restrict__ rec,
     }
     A[tri(r, r)] = kp.diag;
   }
-  T cv[K];
-#pragma unroll
-  for (int j = 0; j < K; ++j) cv[j] = R[j].v;
+}
 
-  // in-place right-looking Cholesky, the values row carried along
+// in-place right-looking Cholesky with the values row cv carried along.
+// On return A holds L below the diagonal, cv = z = L_cc^-1 v_c.  KEEP_INV: A[j][j] = 1 / L_jj (j < K).
+template <typename T, int K, bool KEEP_INV>
+__device__ __forceinline__ Cond<T> factor_joint_reg(T (&A)[(K + 1) * (K + 2) / 2], T (&cv)[K], const KParams<T>& kp) {
   T m = T(0);
   T minpiv = kp.diag;
 #pragma unroll
@@ -93,9 +96,11 @@ __device__ __forceinline__ Cond<T> condition_reg(const Rec<T>* __restrict__ rec,
     T piv = A[tri(j, j)];
     minpiv = Math<T>::fmin(minpiv, piv);
     T inv = Math<T>::rsqrt(piv);
+    if (KEEP_INV) A[tri(j, j)] = inv;
 #pragma unroll
     for (int r = j + 1; r <= K; ++r) A[tri(r, j)] *= inv;
     T zj = cv[j] * inv;
+    cv[j] = zj;
 #pragma unroll
     for (int r = j + 1; r <= K; ++r) {
 #pragma unroll
@@ -112,6 +117,20 @@ __device__ __forceinline__ Cond<T> condition_reg(const Rec<T>* __restrict__ rec,
   out.m = m;
   out.s = Math<T>::sqrt(s2);
   return out;
+}
+
+template <typename T, int K, int D, int KIND, bool COHERENT>
+__device__ __forceinline__ Cond<T> condition_reg(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ row,
+                                                 const Rec<T>& self, const KParams<T>& kp) {
+  int32_t idx[K];
+  Rec<T> R[K];
+  gather_reg<T, K, COHERENT>(rec, row, idx, R);
+  T A[(K + 1) * (K + 2) / 2];
+  build_joint_reg<T, K, D, KIND>(R, self, kp, A);
+  T cv[K];
+#pragma unroll
+  for (int j = 0; j < K; ++j) cv[j] = R[j].v;
+  return factor_joint_reg<T, K, false>(A, cv, kp);
 }
 
 // ---- generic: triangle in shared memory ------------------------------------------------------------

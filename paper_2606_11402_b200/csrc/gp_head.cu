@@ -33,6 +33,28 @@ __global__ void head_build_kernel(const T* __restrict__ x, int d, int n0, int ki
   A[(size_t)r * n0 + c] = val;
 }
 
+// gradient mode: rows n0..2n0-1 = identity, rows 2n0..3n0-1 = ell * dM/dell (symmetric, zero diagonal)
+template <typename T>
+__global__ void head_carry_grad_init_kernel(const T* __restrict__ x, int d, int n0, int kind, KParams<double> kp,
+                                            double* __restrict__ A) {
+  int c = blockIdx.x * blockDim.x + threadIdx.x;
+  int r = blockIdx.y * blockDim.y + threadIdx.y;
+  if (r >= n0 || c >= n0) return;
+  double* C1 = A + (size_t)n0 * n0;
+  double* C2 = C1 + (size_t)n0 * n0;
+  C1[(size_t)r * n0 + c] = r == c ? 1.0 : 0.0;
+  double val = 0.0;
+  if (r != c) {
+    double d2 = 0.0;
+    for (int t = 0; t < d; ++t) {
+      double dx = (double)x[(size_t)r * d + t] - (double)x[(size_t)c * d + t];
+      d2 = fma(dx, dx, d2);
+    }
+    val = drho_rt<double>(kind, d2 * kp.qscale);
+  }
+  C2[(size_t)r * n0 + c] = val;
+}
+
 // carried rows: mode 1 = one row holding src[0:n0]; mode 2 = identity (n0 rows)
 template <typename T>
 __global__ void head_carry_init_kernel(const T* __restrict__ src, int n0, int mode, double* __restrict__ A) {
@@ -162,7 +184,13 @@ gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried) {
   else
     head_build_kernel<float><<<bg, bb, 0, c.st>>>((const float*)c.g->x, c.g->d, n0, c.kern->kind, kp, A);
   GP_LAUNCH_CHECK();
-  if (n_carried > 0) {
+  if (n_carried == 2 * n0 && n_carried > 1) {
+    if (c.g->dtype == GP_F64)
+      head_carry_grad_init_kernel<double><<<bg, bb, 0, c.st>>>((const double*)c.g->x, c.g->d, n0, c.kern->kind, kp, A);
+    else
+      head_carry_grad_init_kernel<float><<<bg, bb, 0, c.st>>>((const float*)c.g->x, c.g->d, n0, c.kern->kind, kp, A);
+    GP_LAUNCH_CHECK();
+  } else if (n_carried > 0) {
     int mode = n_carried == 1 ? 1 : 2;
     int64_t total = mode == 1 ? n0 : (int64_t)n0 * n0;
     unsigned grid = (unsigned)((total + 255) / 256);
@@ -246,10 +274,107 @@ __global__ void head_logdet_kernel(const double* __restrict__ L, int n0, double 
   block_atomic_add(s, acc, red);
 }
 
-gp_status head_logdet(const OpCtx& c, double* acc, double* /*grad_acc*/) {
+// tr(M^-1 D) = sum_{e,b} Linv[e][b] (Linv D)[e][b] = sum over the two carried blocks, element by element
+__global__ void head_trace_kernel(const double* __restrict__ C1, const double* __restrict__ C2, int64_t total, double* acc) {
+  __shared__ double red[32];
+  double s = 0.0;
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < total; e += (int64_t)gridDim.x * blockDim.x)
+    s = fma(C1[e], C2[e], s);
+  block_atomic_add(s, acc, red);
+}
+
+gp_status head_logdet(const OpCtx& c, double* acc, double* grad_ell_acc) {
   const int n0 = (int)c.g->n0;
   if (n0 <= 0) return GP_OK;
   head_logdet_kernel<<<1, 256, 0, c.st>>>(c.head(), n0, c.kern->sigma, acc);
+  GP_LAUNCH_CHECK();
+  if (grad_ell_acc) {
+    const double* C1 = c.head() + (size_t)n0 * n0;
+    const double* C2 = C1 + (size_t)n0 * n0;
+    int64_t total = (int64_t)n0 * n0;
+    unsigned grid = (unsigned)((total + 255) / 256);
+    if (grid > 1184) grid = 1184;
+    head_trace_kernel<<<grid, 256, 0, c.st>>>(C1, C2, total, grad_ell_acc);
+    GP_LAUNCH_CHECK();
+  }
+  return GP_OK;
+}
+
+// ---- VJP through the head:  v_h = sigma L xi_h --------------------------------------------
+//   p = L^T g_h;  xi_bar_h = sigma p;  sigma_bar += g_h . (L xi_h) = p . xi_h
+//   L_bar = sigma tril(g_h xi_h^T);  M_bar = L^-T Phi(L^T L_bar) L^-1, Phi = lower triangle with the diagonal
+//   halved;  L^T L_bar = sigma p xi^T on the lower part.  With T1 = Phi L^-1, i.e.
+//     T1[a][b] = sigma p_a ( sum_{b' <= a} xi_b' Linv[b'][b]  -  xi_a Linv[a][b] / 2 ),
+//   ell_bar = sum_ab M_bar_ab dM_ab/dell = sum_{a,b} T1[a][b] (Linv dM/dell)[a][b]: both factors come out of
+//   the factorisation as carried rows (C1[b][a] = Linv[a][b], C2[b][a] = (Linv D)[a][b]), so no dense
+//   triangular solve or GEMM is needed beyond the factorisation itself.
+template <typename T>
+__global__ void head_vjp_p_kernel(const double* __restrict__ L, const T* __restrict__ gbar, const T* __restrict__ xi,
+                                  T* __restrict__ xibar, double* __restrict__ p, int n0, double sigma, double* acc_sigma) {
+  __shared__ double red[32];
+  int e = blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;   // one warp per column e
+  int lane = threadIdx.x & 31;
+  double contrib = 0.0;
+  if (e < n0) {
+    double s = 0.0;
+    for (int a = e + lane; a < n0; a += 32) s = fma(L[(size_t)a * n0 + e], (double)gbar[a], s);
+    s = warp_sum(s);
+    if (lane == 0) {
+      p[e] = s;
+      xibar[e] = (T)(sigma * s);
+      contrib = s * (double)xi[e];
+    }
+  }
+  block_atomic_add(contrib, acc_sigma, red);
+}
+
+template <typename T>
+__global__ void head_vjp_ell_kernel(const double* __restrict__ C1, const double* __restrict__ C2,
+                                    const double* __restrict__ p, const T* __restrict__ xi, int n0, double sigma,
+                                    double* acc_ell) {
+  __shared__ double red[32];
+  int b = blockIdx.x * (blockDim.x / 32) + threadIdx.x / 32;   // one warp per carried row b
+  int lane = threadIdx.x & 31;
+  double total = 0.0;
+  if (b < n0) {
+    const double* c1 = C1 + (size_t)b * n0;
+    const double* c2 = C2 + (size_t)b * n0;
+    double carry = 0.0;                                         // sum_{a' < chunk} xi_a' Linv[a'][b]
+    for (int a0 = (b / 32) * 32; a0 < n0; a0 += 32) {          // Linv[a][b] = 0 for a < b
+      int a = a0 + lane;
+      double t = a < n0 ? (double)xi[a] * c1[a] : 0.0;
+      double incl = t;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        double up = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += up;
+      }
+      if (a < n0) total = fma(p[a] * (carry + incl - 0.5 * t), c2[a], total);
+      carry += __shfl_sync(0xffffffffu, incl, 31);
+    }
+    total = warp_sum(total);
+    if (lane != 0) total = 0.0;
+  }
+  block_atomic_add(sigma * total, acc_ell, red);
+}
+
+gp_status head_vjp(const OpCtx& c, const void* xi, const void* gbar, void* xibar, double* acc) {
+  const int n0 = (int)c.g->n0;
+  if (n0 <= 0) return GP_OK;
+  const double* L = c.head();
+  const double* C1 = L + (size_t)n0 * n0;
+  const double* C2 = C1 + (size_t)n0 * n0;
+  double* p = c.head() + (size_t)3 * n0 * n0;
+  unsigned grid = (unsigned)((n0 + 3) / 4);
+  if (c.g->dtype == GP_F64) {
+    head_vjp_p_kernel<double><<<grid, 128, 0, c.st>>>(L, (const double*)gbar, (const double*)xi, (double*)xibar, p, n0, c.kern->sigma, acc);
+    GP_LAUNCH_CHECK();
+    head_vjp_ell_kernel<double><<<grid, 128, 0, c.st>>>(C1, C2, p, (const double*)xi, n0, c.kern->sigma, acc + 1);
+  } else {
+    head_vjp_p_kernel<float><<<grid, 128, 0, c.st>>>(L, (const float*)gbar, (const float*)xi, (float*)xibar, p, n0, c.kern->sigma, acc);
+    GP_LAUNCH_CHECK();
+    head_vjp_ell_kernel<float><<<grid, 128, 0, c.st>>>(C1, C2, p, (const float*)xi, n0, c.kern->sigma, acc + 1);
+  }
   GP_LAUNCH_CHECK();
   return GP_OK;
 }

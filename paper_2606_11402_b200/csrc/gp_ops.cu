@@ -182,10 +182,13 @@ static gp_status pack(const OpCtx& c, const T* vals) {
   return GP_OK;
 }
 
-__global__ void finalize_logdet_kernel(const Control* ctrl, double* logdet, double* grad) {
+// grad = d/d(sigma, ell):  every point contributes log sigma^2 + log s_i^2, so d/dsigma = 2 N / sigma exactly;
+// acc[2] holds ell * d/dell (gp_vjp.cu).
+__global__ void finalize_logdet_kernel(const Control* ctrl, double* logdet, double* grad, double two_n_over_sigma,
+                                       double inv_ell) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
     logdet[0] = ctrl->acc[0];
-    if (grad) { grad[0] = ctrl->acc[1]; grad[1] = ctrl->acc[2]; }
+    if (grad) { grad[0] = two_n_over_sigma; grad[1] = ctrl->acc[2] * inv_ell; }
   }
 }
 
@@ -217,10 +220,12 @@ static gp_status logdet_t(const OpCtx& c, double* logdet, double* grad) {
   bool spec = use_spec(c);
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
   if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr));
-  GP_OK_OR_RETURN(head_factor(c, nullptr, 0));
-  GP_OK_OR_RETURN(head_logdet(c, &c.ctrl()->acc[0], nullptr));
+  GP_OK_OR_RETURN(head_factor(c, nullptr, grad ? 2 * (int)c.g->n0 : 0));
+  GP_OK_OR_RETURN(head_logdet(c, &c.ctrl()->acc[0], grad ? &c.ctrl()->acc[2] : nullptr));
   GP_OK_OR_RETURN((launch_range<T, OPK_LOGDET>(c, spec, nullptr, nullptr, nullptr, c.g->n0, c.g->n)));
-  finalize_logdet_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), logdet, grad);
+  if (grad) GP_OK_OR_RETURN(run_logdet_grad(c));
+  finalize_logdet_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), logdet, grad, 2.0 * (double)c.g->n / c.kern->sigma,
+                                             1.0 / c.kern->ell);
   GP_LAUNCH_CHECK();
   return GP_OK;
 }

@@ -1,6 +1,314 @@
-// placeholder, replaced below
+// Kernel-parameter derivatives ("backward derivatives"):
+//   gp_vjp     VJP of the forward map (xi, sigma, ell) -> v for a cotangent v_bar
+//   gp_logdet  gradient d/d(sigma, ell) of sum_i log s_i^2
+//
+// Per point, in unit-sigma form M = K / sigma^2 with joint factor L (Alg. 1):
+//   l = L[k][0:k], s = L[k][k], z = L_cc^-1 v_c,   v_i = l.z + sigma s xi_i
+//   w = L_cc^-T l  (= K_cc^-1 K_ci),  alpha = L_cc^-T z  (= M_cc^-1 v_c),  u = (-w, 1)
+//   y = (dM/dell) u  where dM_ab/dell = drho/dell(r_ab), zero on the diagonal
+// For the total cotangent g on v_i (all later batches already scattered into it):
+//   xi_bar_i   = g sigma s
+//   g_c       += g w                                     (k floating-point atomics)
+//   sigma_bar += g s xi_i                                (v_i depends on sigma only through sigma s xi_i)
+//   ell_bar   += g ( y[0:k].alpha + sigma xi_i (y.u) / (2 s) )
+// and for the log-determinant  d/dell log s_i^2 = (y.u) / s^2,  d/dsigma sum_i log(sigma^2 s_i^2) = 2 N / sigma.
+// These are the differentials dm = u^T dM [alpha; 0], d(s^2) = u^T dM u of Eq. 2 (R-14); the oracle
+// reaches the same numbers by summing K_bar_ab dK_ab/dtheta over the full joint matrix in the solve form.
+//
+// Batches run in REVERSE order (one launch per batch): a point's cotangent is complete once every later
+// batch has scattered into it, and points of one batch never touch each other's cotangent.
+#include <type_traits>
+
 #include "gp_cond.cuh"
+
 namespace gp {
-gp_status run_vjp(const OpCtx&, const void*, const void*, const void*, void*, double*) { return GP_ERR_UNSUPPORTED; }
-gp_status head_vjp(const OpCtx&, const void*, const void*, void*, double*) { return GP_ERR_UNSUPPORTED; }
+
+enum { GRAD_VJP = 0, GRAD_LOGDET = 1 };
+constexpr int kGradThreads = 128;
+
+template <typename T> __device__ __forceinline__ T qnan();
+template <> __device__ __forceinline__ float qnan<float>() { return __int_as_float(0x7fc00000); }
+template <> __device__ __forceinline__ double qnan<double>() { return __longlong_as_double(0x7ff8000000000000LL); }
+
+// rec[i] = {x_i, vals_i or 0}  (same packed record the forward kernels gather)
+template <typename T>
+__global__ void grad_pack_kernel(const T* __restrict__ x, const T* __restrict__ vals, Rec<T>* __restrict__ rec,
+                                 int64_t n, int d) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  Rec<T> r;
+  r.x0 = x[i * d];
+  r.x1 = d >= 2 ? x[i * d + 1] : T(0);
+  r.x2 = d >= 3 ? x[i * d + 2] : T(0);
+  r.v = vals ? vals[i] : T(0);
+  rec[i] = r;
 }
+
+// ---- register-resident gradient kernel -----------------------------------------------------------------
+template <typename T, int K, int D, int KIND, int MODE>
+__global__ void __launch_bounds__(kGradThreads)
+grad_kernel(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* __restrict__ xi,
+            T* gbar, T* __restrict__ xibar, int64_t start, int64_t end, int64_t n0, KParams<T> kp, Control* ctrl) {
+  __shared__ double red[32];
+  int64_t i = start + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  double acc_sigma = 0.0, acc_ell = 0.0;
+  if (i < end) {
+    Rec<T> self = load_rec<false>(rec + i);
+    int32_t idx[K];
+    Rec<T> R[K];
+    gather_reg<T, K, false>(rec, nbr + (i - n0) * K, idx, R);
+    constexpr int NT = (K + 1) * (K + 2) / 2;
+    T A[NT];
+    build_joint_reg<T, K, D, KIND>(R, self, kp, A);
+    T cv[K];
+#pragma unroll
+    for (int j = 0; j < K; ++j) cv[j] = R[j].v;
+    Cond<T> c = factor_joint_reg<T, K, true>(A, cv, kp);
+    // back-substitution, in place:  A[K][j] <- w_j,  cv[j] <- alpha_j
+#pragma unroll
+    for (int j = K - 1; j >= 0; --j) {
+      T w = A[tri(K, j)], a = cv[j];
+#pragma unroll
+      for (int r = j + 1; r < K; ++r) {
+        w = Math<T>::fma(-A[tri(r, j)], A[tri(K, r)], w);
+        a = Math<T>::fma(-A[tri(r, j)], cv[r], a);
+      }
+      A[tri(K, j)] = w * A[tri(j, j)];
+      cv[j] = a * A[tri(j, j)];
+    }
+    // y = (ell dM/dell) u, u = (-w, 1); the triangle of L_cc is dead from here on
+    T y[K + 1];
+#pragma unroll
+    for (int j = 0; j <= K; ++j) y[j] = T(0);
+#pragma unroll
+    for (int r = 1; r <= K; ++r) {
+      T ur = (r == K) ? T(1) : -A[tri(K, r)];
+#pragma unroll
+      for (int cc = 0; cc < r; ++cc) {
+        T q = (r == K) ? pair_q<T, D>(self, R[cc], kp.qscale) : pair_q<T, D>(R[r], R[cc], kp.qscale);
+        T dq = Math<T>::template drho_from_q<KIND>(q);
+        y[r] = Math<T>::fma(-dq, A[tri(K, cc)], y[r]);   // dq * u_cc
+        y[cc] = Math<T>::fma(dq, ur, y[cc]);
+      }
+    }
+    T yu = y[K], ya = T(0);
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+      yu = Math<T>::fma(-y[j], A[tri(K, j)], yu);
+      ya = Math<T>::fma(y[j], cv[j], ya);
+    }
+    if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
+    if (MODE == GRAD_VJP) {
+      T g = gbar[i];
+      T xi_i = xi[i];
+      T gs = g * c.s;
+      T out = kp.sigma * gs;
+      if (!c.ok) out = qnan<T>();
+      xibar[i] = out;
+      if (c.ok) {
+#pragma unroll
+        for (int j = 0; j < K; ++j) atomicAdd(gbar + idx[j], g * A[tri(K, j)]);
+        acc_sigma = (double)(gs * xi_i);
+        acc_ell = (double)(g * (ya + T(0.5) * kp.sigma * xi_i * yu / c.s));
+      }
+    } else {
+      if (c.ok) acc_ell = (double)(yu / (c.s * c.s));
+    }
+  }
+  if (MODE == GRAD_VJP) block_atomic_add(acc_sigma, &ctrl->acc[3], red);
+  block_atomic_add(acc_ell, &ctrl->acc[MODE == GRAD_VJP ? 4 : 2], red);
+}
+
+// ---- generic gradient kernel: triangle in shared memory, any k <= 64, d <= 4 -----------------------------
+template <typename T, int MODE>
+__global__ void grad_generic_kernel(const T* __restrict__ x, const T* __restrict__ vals, const int32_t* __restrict__ nbr,
+                                    const T* __restrict__ xi, T* gbar, T* __restrict__ xibar, int64_t start, int64_t end,
+                                    int64_t n0, int d, int k, int kind, KParams<T> kp, Control* ctrl, int active) {
+  extern __shared__ double smem_raw[];
+  __shared__ double red[32];
+  int tid = threadIdx.x;
+  int64_t i = start + (int64_t)blockIdx.x * active + tid;
+  double acc_sigma = 0.0, acc_ell = 0.0;
+  if (tid < active && i < end) {
+    Scratch<T> A{reinterpret_cast<T*>(smem_raw) + tid, active};
+    const int32_t* row = nbr + (i - n0) * k;
+    const int NT = (k + 1) * (k + 2) / 2;
+    Cond<T> c = condition_generic<T>(x, MODE == GRAD_VJP ? vals : nullptr, d, k, kind, row, i, kp, A);
+    // back-substitution: A[k][j] <- w_j, A[NT + j] <- alpha_j   (A[j][j] = L_jj)
+    for (int j = k - 1; j >= 0; --j) {
+      T w = A[tri(k, j)], a = A[NT + j];
+      for (int r = j + 1; r < k; ++r) {
+        T lrj = A[tri(r, j)];
+        w = Math<T>::fma(-lrj, A[tri(k, r)], w);
+        a = Math<T>::fma(-lrj, A[NT + r], a);
+      }
+      T inv = T(1) / A[tri(j, j)];
+      A[tri(k, j)] = w * inv;
+      A[NT + j] = a * inv;
+    }
+    const int YO = NT + k;
+    for (int j = 0; j <= k; ++j) A[YO + j] = T(0);
+    for (int r = 1; r <= k; ++r) {
+      int64_t pr = (r == k) ? i : (int64_t)row[r];
+      T ur = (r == k) ? T(1) : -A[tri(k, r)];
+      T yr = T(0);
+      for (int cc = 0; cc < r; ++cc) {
+        T dq = drho_rt<T>(kind, dist_q<T>(x, d, pr, (int64_t)row[cc], kp.qscale));
+        yr = Math<T>::fma(-dq, A[tri(k, cc)], yr);
+        A[YO + cc] = Math<T>::fma(dq, ur, A[YO + cc]);
+      }
+      A[YO + r] += yr;
+    }
+    T yu = A[YO + k], ya = T(0);
+    for (int j = 0; j < k; ++j) {
+      yu = Math<T>::fma(-A[YO + j], A[tri(k, j)], yu);
+      ya = Math<T>::fma(A[YO + j], A[NT + j], ya);
+    }
+    if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
+    if (MODE == GRAD_VJP) {
+      T g = gbar[i];
+      T xi_i = xi[i];
+      T gs = g * c.s;
+      T out = kp.sigma * gs;
+      if (!c.ok) out = qnan<T>();
+      xibar[i] = out;
+      if (c.ok) {
+        for (int j = 0; j < k; ++j) atomicAdd(gbar + row[j], g * A[tri(k, j)]);
+        acc_sigma = (double)(gs * xi_i);
+        acc_ell = (double)(g * (ya + T(0.5) * kp.sigma * xi_i * yu / c.s));
+      }
+    } else {
+      if (c.ok) acc_ell = (double)(yu / (c.s * c.s));
+    }
+  }
+  if (MODE == GRAD_VJP) block_atomic_add(acc_sigma, &ctrl->acc[3], red);
+  block_atomic_add(acc_ell, &ctrl->acc[MODE == GRAD_VJP ? 4 : 2], red);
+}
+
+// ---- host side --------------------------------------------------------------------------------------------
+int generic_active_threads(int k, size_t elem_bytes, bool with_vjp);   // gp_ops.cu
+
+// fp64 gradients go through the shared-memory kernel: with 2 x 36 inlined double exp/sqrt the register-resident
+// form makes ptxas fall back to a spill-everything allocation (32 registers, 7 KB of local memory per thread).
+#define GP_GRAD_SPEC_TABLE(X) X(float, 8, 3) X(float, 16, 3) X(float, 8, 2) X(float, 16, 2)
+
+template <typename T, int K, int D, int MODE>
+static gp_status launch_grad_spec(const OpCtx& c, const T* xi, T* gbar, T* xibar, int64_t start, int64_t end) {
+  int64_t cnt = end - start;
+  if (cnt <= 0) return GP_OK;
+  unsigned grid = (unsigned)((cnt + kGradThreads - 1) / kGradThreads);
+  KParams<T> kp = make_kparams<T>(*c.kern);
+  const Rec<T>* rec = (const Rec<T>*)c.rec();
+  switch (c.kern->kind) {
+    case GP_KERNEL_SE:
+      grad_kernel<T, K, D, GP_KERNEL_SE, MODE><<<grid, kGradThreads, 0, c.st>>>(rec, c.g->nbr, xi, gbar, xibar, start, end, c.g->n0, kp, c.ctrl());
+      break;
+    case GP_KERNEL_MATERN32:
+      grad_kernel<T, K, D, GP_KERNEL_MATERN32, MODE><<<grid, kGradThreads, 0, c.st>>>(rec, c.g->nbr, xi, gbar, xibar, start, end, c.g->n0, kp, c.ctrl());
+      break;
+    default:
+      grad_kernel<T, K, D, GP_KERNEL_EXP, MODE><<<grid, kGradThreads, 0, c.st>>>(rec, c.g->nbr, xi, gbar, xibar, start, end, c.g->n0, kp, c.ctrl());
+      break;
+  }
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+template <typename T, int MODE>
+static gp_status launch_grad_generic(const OpCtx& c, const T* vals, const T* xi, T* gbar, T* xibar, int64_t start,
+                                     int64_t end) {
+  int64_t cnt = end - start;
+  if (cnt <= 0) return GP_OK;
+  int k = c.g->k;
+  int active = generic_active_threads(k, sizeof(T), true);
+  int threads = (active + 31) / 32 * 32;
+  size_t smem = (size_t)generic_scratch_elems(k, true) * sizeof(T) * active;
+  static bool attr_set = false;
+  if (!attr_set) {
+    GP_CUDA_OK(cudaFuncSetAttribute(grad_generic_kernel<T, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
+    attr_set = true;
+  }
+  unsigned grid = (unsigned)((cnt + active - 1) / active);
+  KParams<T> kp = make_kparams<T>(*c.kern);
+  grad_generic_kernel<T, MODE><<<grid, threads, smem, c.st>>>((const T*)c.g->x, vals, c.g->nbr, xi, gbar, xibar, start, end,
+                                                            c.g->n0, c.g->d, k, c.kern->kind, kp, c.ctrl(), active);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+static bool grad_use_spec(const OpCtx& c) {
+  if (c.g->flags & GP_FLAG_GENERIC_KERNEL) return false;
+  bool have = false;
+#define X(T, K, D) \
+  if ((c.g->dtype == GP_F64) == (sizeof(T) == 8) && c.g->k == K && c.g->d == D) have = true;
+  GP_GRAD_SPEC_TABLE(X)
+#undef X
+  return have && (((uintptr_t)c.g->nbr) & 15) == 0;
+}
+
+template <typename T, int MODE>
+static gp_status launch_grad_range(const OpCtx& c, bool spec, const T* vals, const T* xi, T* gbar, T* xibar,
+                                   int64_t start, int64_t end) {
+  if (spec) {
+#define X(TT, K, D) \
+    if constexpr (std::is_same<TT, T>::value) {                    \
+      if (c.g->k == K && c.g->d == D) return launch_grad_spec<T, K, D, MODE>(c, xi, gbar, xibar, start, end); \
+    }
+    GP_GRAD_SPEC_TABLE(X)
+#undef X
+  }
+  return launch_grad_generic<T, MODE>(c, vals, xi, gbar, xibar, start, end);
+}
+
+template <typename T>
+static gp_status grad_pack(const OpCtx& c, const T* vals) {
+  int64_t n = c.g->n;
+  grad_pack_kernel<T><<<(unsigned)((n + 255) / 256), 256, 0, c.st>>>((const T*)c.g->x, vals, (Rec<T>*)c.rec(), n, c.g->d);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+// theta_bar[0] = sigma_bar, theta_bar[1] = ell_bar; the kernels accumulate ell * d/dell
+__global__ void finalize_grad_kernel(const Control* ctrl, int slot_sigma, int slot_ell, double inv_ell, double* out2) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) {
+    out2[0] = ctrl->acc[slot_sigma];
+    out2[1] = ctrl->acc[slot_ell] * inv_ell;
+  }
+}
+
+template <typename T>
+static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T* xibar, double* thetabar) {
+  bool spec = grad_use_spec(c);
+  const int64_t n = c.g->n, n0 = c.g->n0;
+  T* gbar = (T*)c.gbar();
+  GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
+  GP_CUDA_OK(cudaMemcpyAsync(gbar, vbar, (size_t)n * sizeof(T), cudaMemcpyDeviceToDevice, c.st));
+  if (spec) GP_OK_OR_RETURN(grad_pack<T>(c, v));
+  const int64_t* off = c.g->batch_off;
+  for (int b = c.g->n_batches - 1; b >= 0; --b)
+    GP_OK_OR_RETURN((launch_grad_range<T, GRAD_VJP>(c, spec, v, xi, gbar, xibar, off[b], off[b + 1])));
+  if (n0 > 0) {
+    GP_OK_OR_RETURN(head_factor(c, nullptr, 2 * (int)n0));
+    GP_OK_OR_RETURN(head_vjp(c, xi, gbar, xibar, &c.ctrl()->acc[3]));
+  }
+  finalize_grad_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), 3, 4, 1.0 / c.kern->ell, thetabar);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+gp_status run_vjp(const OpCtx& c, const void* xi, const void* v, const void* vbar, void* xibar, double* thetabar) {
+  return c.g->dtype == GP_F64 ? vjp_t<double>(c, (const double*)xi, (const double*)v, (const double*)vbar, (double*)xibar, thetabar)
+                              : vjp_t<float>(c, (const float*)xi, (const float*)v, (const float*)vbar, (float*)xibar, thetabar);
+}
+
+// gradient of the log-determinant: acc[1] = d/dsigma, acc[2] = ell * d/dell (conditioning part)
+template <typename T>
+static gp_status logdet_grad_t(const OpCtx& c) {
+  bool spec = grad_use_spec(c);
+  return launch_grad_range<T, GRAD_LOGDET>(c, spec, nullptr, nullptr, nullptr, nullptr, c.g->n0, c.g->n);
+}
+gp_status run_logdet_grad(const OpCtx& c) {
+  return c.g->dtype == GP_F64 ? logdet_grad_t<double>(c) : logdet_grad_t<float>(c);
+}
+
+}  // namespace gp
