@@ -208,8 +208,10 @@ def run_graft(args):
     xi_back = torch.empty_like(xi)
     st = torch.cuda.current_stream()
 
-    ops = ["forward", "inverse", "logdet", "vjp"]
+    ops = [o for o in ("forward", "inverse", "logdet", "vjp") if o in args.ops.split(",")]
     state = {}
+    if "forward" not in ops:      # the other ops need a v to work on
+        gp.gp_forward(G, K, xi, out=v)
 
     def do(op):
         if op == "forward":
@@ -225,7 +227,7 @@ def run_graft(args):
         for op in ops:
             do(op)
     torch.cuda.synchronize()
-    for op in ("forward", "inverse", "logdet", "vjp"):
+    for op in ops:
         nbad = gp.check_errors(G.workspace({"forward": gp.GP_OP_FORWARD, "inverse": gp.GP_OP_INVERSE,
                                             "logdet": gp.GP_OP_LOGDET, "vjp": gp.GP_OP_VJP}[op]))
         if nbad:
@@ -270,11 +272,17 @@ def run_graft(args):
     ld_p = torch.empty(1, dtype=torch.float64).pin_memory()
     staging = (in_dev, out_dev, torch.empty_like(xi), torch.empty_like(xi), torch.empty(2, dtype=torch.float64, device=dev))
 
+    v_p.copy_(v)
+
     def e2e_step():
-        gp.gp_forward_host(G, K, xi_p, v_p, in_dev, out_dev)
-        gp.gp_inverse_host(G, K, v_p, xi2_p, in_dev, out_dev)
-        ld_p.copy_(gp.gp_logdet(G, K), non_blocking=True)
-        gp.gp_vjp_host(G, K, xi_p, v_p, vbar_p, xib_p, tb_p, staging)
+        if "forward" in ops:
+            gp.gp_forward_host(G, K, xi_p, v_p, in_dev, out_dev)
+        if "inverse" in ops:
+            gp.gp_inverse_host(G, K, v_p, xi2_p, in_dev, out_dev)
+        if "logdet" in ops:
+            ld_p.copy_(gp.gp_logdet(G, K), non_blocking=True)
+        if "vjp" in ops:
+            gp.gp_vjp_host(G, K, xi_p, v_p, vbar_p, xib_p, tb_p, staging)
 
     e2e_step()
     torch.cuda.synchronize()
@@ -291,8 +299,9 @@ def run_graft(args):
         t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_ms = float(t.item())
-    h2d = n * B * (1 + 1 + 3)          # forward xi; inverse v; vjp xi, v, v_bar
-    d2h = n * B * 3 + 8 + 16           # v; xi; xi_bar; logdet; theta_bar
+    # forward xi -> v; inverse v -> xi; logdet -> 8 B; vjp xi, v, v_bar -> xi_bar, theta_bar
+    h2d = n * B * sum({"forward": 1, "inverse": 1, "logdet": 0, "vjp": 3}[o] for o in ops)
+    d2h = sum({"forward": n * B, "inverse": n * B, "logdet": 8, "vjp": n * B + 16}[o] for o in ops)
 
     if rank != 0:
         return
@@ -307,8 +316,7 @@ def run_graft(args):
         ops_out[op] = dict(ms=round(op_ms[op], 4), points_per_s=n / t_s, flop_per_point=flop, bytes_per_point=byt,
                            tflops=flop * npts / t_s / 1e12, gbs=byt * npts / t_s / 1e9,
                            roofline_frac=max(t_alu, t_hbm) / t_s, bound="alu" if t_alu >= t_hbm else "hbm")
-    f = ops_out["forward"]
-    flop, byt = algorithmic_work(cfg.k, cfg.d, cfg.kind, B, "forward")
+    f = ops_out["forward" if "forward" in ops else ops[0]]
     if f["bound"] == "alu":
         roof = dict(bound="alu", achieved=f["tflops"], peak=alu_peak, unit="TFLOP/s", frac=f["tflops"] / alu_peak,
                     traffic=None, peak_source="nominal non-tensor peak, 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz",
@@ -323,7 +331,7 @@ def run_graft(args):
         "dtype": dtype, "data": "synthetic",
         "config": {"workload": f"config {cfg.cid}: {cfg.name}, N={n}, d={cfg.d}, k={cfg.k}, n0={cfg.n0}, "
                                f"{cfg.kind} sigma={cfg.sigma} ell={cfg.ell} jitter={cfg.jitter}",
-                   "step": "gp_forward + gp_inverse + gp_logdet + gp_vjp, each over all N points",
+                   "step": " + ".join("gp_" + o for o in ops) + ", each over all N points",
                    "n_batches": L, "parallelism": "replicas" if world > 1 else "single GPU",
                    "l2": "inputs larger than L2 (nbr %.0f MiB + records %.0f MiB per op)" % (
                        npts * cfg.k * 4 / 2 ** 20, n * 4 * B / 2 ** 20)},
@@ -401,6 +409,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configuration (1-5); 3 = the headline")
     ap.add_argument("--n", type=int, default=0, help="override the number of points (smaller dry runs)")
     ap.add_argument("--dtype", default="", choices=["", "f32", "f64"])
+    ap.add_argument("--ops", default="forward,inverse,logdet,vjp", help="subset of the step to run (profiling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--reference-points", type=int, default=1 << 16)
