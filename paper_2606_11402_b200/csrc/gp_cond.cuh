@@ -30,6 +30,20 @@ template <bool COHERENT> __device__ __forceinline__ Rec<double> load_rec(const R
   Rec<double> r; r.x0 = a.x; r.x1 = a.y; r.x2 = b.x; r.v = b.y; return r;
 }
 
+// Ordinary (L1-allocating) load of a record that a CTA of the same launch may still be writing: the
+// coordinates never change, and the value word is either "pending" or final (see forward_flow_kernel).
+__device__ __forceinline__ Rec<float> load_rec_l1(const Rec<float>* p) {
+  float4 t;
+  asm volatile("ld.global.ca.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(t.x), "=f"(t.y), "=f"(t.z), "=f"(t.w) : "l"(p));
+  Rec<float> r; r.x0 = t.x; r.x1 = t.y; r.x2 = t.z; r.v = t.w; return r;
+}
+__device__ __forceinline__ Rec<double> load_rec_l1(const Rec<double>* p) {
+  double a, b, c, d;
+  asm volatile("ld.global.ca.v2.f64 {%0, %1}, [%2];" : "=d"(a), "=d"(b) : "l"(p));
+  asm volatile("ld.global.ca.v2.f64 {%0, %1}, [%2];" : "=d"(c), "=d"(d) : "l"(reinterpret_cast<const double*>(p) + 2));
+  Rec<double> r; r.x0 = a; r.x1 = b; r.x2 = c; r.v = d; return r;
+}
+
 template <typename T, int D> __device__ __forceinline__ T pair_q(const Rec<T>& a, const Rec<T>& b, T qscale) {
   T dx = a.x0 - b.x0;
   T d2 = dx * dx;
@@ -87,7 +101,7 @@ __device__ __forceinline__ void build_joint_reg(const Rec<T> (&R)[K], const Rec<
 
 // in-place right-looking Cholesky with the values row cv carried along.
 // On return A holds L below the diagonal, cv = z = L_cc^-1 v_c.  KEEP_INV: A[j][j] = 1 / L_jj (j < K).
-template <typename T, int K, bool KEEP_INV>
+template <typename T, int K, bool KEEP_INV, bool CARRY = true>
 __device__ __forceinline__ Cond<T> factor_joint_reg(T (&A)[(K + 1) * (K + 2) / 2], T (&cv)[K], const KParams<T>& kp) {
   T m = T(0);
   T minpiv = kp.diag;
@@ -99,16 +113,18 @@ __device__ __forceinline__ Cond<T> factor_joint_reg(T (&A)[(K + 1) * (K + 2) / 2
     if (KEEP_INV) A[tri(j, j)] = inv;
 #pragma unroll
     for (int r = j + 1; r <= K; ++r) A[tri(r, j)] *= inv;
-    T zj = cv[j] * inv;
-    cv[j] = zj;
+    T zj = T(0);
+    if (CARRY) { zj = cv[j] * inv; cv[j] = zj; }
 #pragma unroll
     for (int r = j + 1; r <= K; ++r) {
 #pragma unroll
       for (int c = j + 1; c <= r; ++c) A[tri(r, c)] = Math<T>::fma(-A[tri(r, j)], A[tri(c, j)], A[tri(r, c)]);
     }
+    if (CARRY) {
 #pragma unroll
-    for (int c = j + 1; c < K; ++c) cv[c] = Math<T>::fma(-zj, A[tri(c, j)], cv[c]);
-    m = Math<T>::fma(zj, A[tri(K, j)], m);
+      for (int c = j + 1; c < K; ++c) cv[c] = Math<T>::fma(-zj, A[tri(c, j)], cv[c]);
+      m = Math<T>::fma(zj, A[tri(K, j)], m);
+    }
   }
   T s2 = A[tri(K, K)];
   minpiv = Math<T>::fmin(minpiv, s2);
@@ -131,6 +147,25 @@ __device__ __forceinline__ Cond<T> condition_reg(const Rec<T>* __restrict__ rec,
 #pragma unroll
   for (int j = 0; j < K; ++j) cv[j] = R[j].v;
   return factor_joint_reg<T, K, false>(A, cv, kp);
+}
+
+// v-independent half of the conditioning (dataflow forward): factor the joint matrix WITHOUT a carried values
+// row, then back-substitute  w = L_cc^-T l  (= K_cc^-1 K_ci, Eq. 2), so that all that is left once the
+// neighbour values exist is the dot product  m = w . v_c.
+template <typename T, int K, int D, int KIND>
+__device__ __forceinline__ Cond<T> weights_reg(const Rec<T> (&R)[K], const Rec<T>& self, const KParams<T>& kp,
+                                               T (&w)[K]) {
+  T A[(K + 1) * (K + 2) / 2];
+  build_joint_reg<T, K, D, KIND>(R, self, kp, A);
+  Cond<T> c = factor_joint_reg<T, K, true, false>(A, w, kp);
+#pragma unroll
+  for (int j = K - 1; j >= 0; --j) {
+    T t = A[tri(K, j)];
+#pragma unroll
+    for (int r = j + 1; r < K; ++r) t = Math<T>::fma(-A[tri(r, j)], w[r], t);
+    w[j] = t * A[tri(j, j)];
+  }
+  return c;
 }
 
 // ---- generic: triangle in shared memory ------------------------------------------------------------

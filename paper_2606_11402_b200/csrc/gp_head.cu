@@ -7,7 +7,11 @@
 // a carried row that starts as r^T ends as (L^-1 r)^T, exactly the values row of Alg. 1.
 //   inverse : 1 carried row  = v_head^T      ->  (L^-1 v_head)^T = sigma * xi_head^T
 //   VJP     : n0 carried rows = identity     ->  L^-T
+#include <cooperative_groups.h>
+
 #include "gp_cond.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace gp {
 
@@ -66,110 +70,146 @@ __global__ void head_carry_init_kernel(const T* __restrict__ src, int n0, int mo
   else C[e] = (e / n0 == e % n0) ? 1.0 : 0.0;
 }
 
-// One block column: every CTA factors the nb x nb diagonal block in shared memory (redundantly — it is
-// tiny), CTA 0 writes it back, and each thread then solves one row of the panel below against it.
-__global__ void __launch_bounds__(64)
-head_panel_kernel(double* __restrict__ A, int n0, int rows_total, int j0, Control* ctrl) {
+// The whole blocked factorisation in ONE cooperative launch (the per-panel launches of a host loop cost more
+// than the arithmetic: n0 = 1024 is 32 panels, each a strictly serial step).  Per panel two grid barriers:
+//   phase 1  every CTA that owns panel rows factors the 32 x 32 diagonal block (one warp, rows in registers,
+//            pivots broadcast by shuffles), CTA 0 writes it back, then one thread per row solves its panel row;
+//   phase 2  64 x 64 trailing tiles, dealt round-robin to the CTAs.
+__device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
+
+// Pivot J of the in-register 32 x 32 factorisation (lane r holds row r); a template recursion so that every
+// index into a[] is a compile-time constant (a loop this size is not unrolled reliably -> local memory).
+template <int J> struct DiagStep {
+  static __device__ __forceinline__ void run(double (&a)[NB], int lane, double* invd, bool& bad) {
+    double piv = shfl_d(a[J], J);
+    bad |= !(piv > 0.0);
+    double inv = rsqrt(piv);
+    inv = inv * fma(-0.5 * piv * inv, inv, 1.5);     // one Newton step: full double accuracy
+    double lj = a[J] * inv;                           // lane J: sqrt(piv); lanes > J: L[lane][J]
+    a[J] = lj;
+    if (lane == J) invd[J] = inv;
+#pragma unroll
+    for (int c = J + 1; c < NB; ++c) {
+      double lc = shfl_d(lj, c);
+      a[c] = fma(-lj, lane >= c ? lc : 0.0, a[c]);
+    }
+    DiagStep<J + 1>::run(a, lane, invd, bad);
+  }
+};
+template <> struct DiagStep<NB> {
+  static __device__ __forceinline__ void run(double (&)[NB], int, double*, bool&) {}
+};
+
+__global__ void __launch_bounds__(256)
+head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) {
+  cg::grid_group grid = cg::this_grid();
   __shared__ double Ds[NB][NB + 1];
   __shared__ double invd[NB];
-  const int nb = min(NB, n0 - j0);
-  const int tid = threadIdx.x;
-  for (int e = tid; e < NB * NB; e += blockDim.x) {
-    int r = e / NB, c = e % NB;
-    Ds[r][c] = (r < nb && c <= r) ? A[(size_t)(j0 + r) * n0 + j0 + c] : (r == c ? 1.0 : 0.0);
-  }
-  __syncthreads();
-  if (tid < 32) {
-    const int lane = tid;
-    for (int j = 0; j < nb; ++j) {
-      if (lane == j) {
-        double piv = Ds[j][j];
-        if (!(piv > 0.0) && blockIdx.x == 0) atomicAdd(&ctrl->n_bad, 1ULL);
-        double sq = sqrt(piv);
-        Ds[j][j] = sq;
-        invd[j] = 1.0 / sq;
-      }
-      __syncwarp();
-      if (lane > j && lane < nb) {
-        double l = Ds[lane][j] * invd[j];
-        Ds[lane][j] = l;
-      }
-      __syncwarp();
-      if (lane > j && lane < nb) {
-        double l = Ds[lane][j];
-        for (int c = j + 1; c <= lane; ++c) Ds[lane][c] = fma(-l, Ds[c][j], Ds[lane][c]);
-      }
-      __syncwarp();
-    }
-  }
-  __syncthreads();
-  if (blockIdx.x == 0) {
-    for (int e = tid; e < nb * nb; e += blockDim.x) {
-      int r = e / nb, c = e % nb;
-      if (c <= r) A[(size_t)(j0 + r) * n0 + j0 + c] = Ds[r][c];
-    }
-  }
-  int r = j0 + nb + blockIdx.x * blockDim.x + tid;
-  if (r >= rows_total) return;
-  double* arow = A + (size_t)r * n0 + j0;
-  double a[NB];
-#pragma unroll
-  for (int c = 0; c < NB; ++c) a[c] = (c < nb) ? arow[c] : 0.0;
-#pragma unroll
-  for (int c = 0; c < NB; ++c) {
-    double acc = a[c];
-#pragma unroll
-    for (int t = 0; t < c; ++t) acc = fma(-a[t], Ds[c][t], acc);
-    a[c] = (c < nb) ? acc * invd[c] : 0.0;
-  }
-#pragma unroll
-  for (int c = 0; c < NB; ++c)
-    if (c < nb) arow[c] = a[c];
-}
-
-// Trailing update  A[r][c] -= sum_t P[r][t] P[c][t]  for r >= j1 = j0 + nb, j1 <= c <= min(r, n0 - 1).
-__global__ void __launch_bounds__(256)
-head_update_kernel(double* __restrict__ A, int n0, int rows_total, int j0, int nb) {
   __shared__ double Pr[NB][64 + 2];
   __shared__ double Pc[NB][64 + 2];
-  const int j1 = j0 + nb;
-  const int r0 = j1 + blockIdx.y * 64, c0 = j1 + blockIdx.x * 64;
-  if (c0 >= n0 || r0 >= rows_total) return;
-  if (r0 < n0 && c0 > r0 + 63) return;   // tile entirely above the diagonal of the square part
-  const int tid = threadIdx.x;
-  for (int e = tid; e < 64 * NB; e += 256) {
-    int row = e / NB, t = e % NB;
-    int rr = r0 + row, cc = c0 + row;
-    Pr[t][row] = (rr < rows_total && t < nb) ? A[(size_t)rr * n0 + j0 + t] : 0.0;
-    Pc[t][row] = (cc < n0 && t < nb) ? A[(size_t)cc * n0 + j0 + t] : 0.0;
-  }
-  __syncthreads();
-  const int tx = tid % 16, ty = tid / 16;
-  double acc[4][4];
+  const int tid = threadIdx.x, lane = tid & 31;
+  const int G = gridDim.x;
+  for (int j0 = 0; j0 < n0; j0 += NB) {
+    const int nb = min(NB, n0 - j0);
+    const int j1 = j0 + nb;
+    const int below = rows_total - j1;
+    // ---- phase 1 --------------------------------------------------------------------------------------
+    const int per = (below + G - 1) / G;                  // panel rows per CTA (<= 256 for every size allowed)
+    const int r_begin = j1 + (int)blockIdx.x * per;
+    const int my_rows = max(0, min(per, rows_total - r_begin));
+    if (my_rows > 0 || blockIdx.x == 0) {
+      if (tid < 32) {
+        double a[NB];
 #pragma unroll
-  for (int a = 0; a < 4; ++a)
+        for (int c = 0; c < NB; ++c)
+          a[c] = (lane < nb && c <= lane && c < nb) ? A[(size_t)(j0 + lane) * n0 + j0 + c] : (c == lane ? 1.0 : 0.0);
+        bool bad = false;
+        DiagStep<0>::run(a, lane, invd, bad);
+        if (bad && blockIdx.x == 0 && lane == 0) atomicAdd(&ctrl->n_bad, 1ULL);
 #pragma unroll
-    for (int b = 0; b < 4; ++b) acc[a][b] = 0.0;
-#pragma unroll 8
-  for (int t = 0; t < NB; ++t) {
-    double pr[4], pc[4];
+        for (int c = 0; c < NB; ++c) {
+          Ds[lane][c] = a[c];
+          if (blockIdx.x == 0 && lane < nb && c <= lane) A[(size_t)(j0 + lane) * n0 + j0 + c] = a[c];
+        }
+      }
+      __syncthreads();
+      if (tid < my_rows) {
+        double* arow = A + (size_t)(r_begin + tid) * n0 + j0;
+        double a[NB];
 #pragma unroll
-    for (int a = 0; a < 4; ++a) { pr[a] = Pr[t][ty * 4 + a]; pc[a] = Pc[t][tx * 4 + a]; }
+        for (int c = 0; c < NB; ++c) a[c] = (c < nb) ? arow[c] : 0.0;
 #pragma unroll
-    for (int a = 0; a < 4; ++a)
+        for (int c = 0; c < NB; ++c) {
+          double v = a[c] * invd[c];
+          a[c] = v;
 #pragma unroll
-      for (int b = 0; b < 4; ++b) acc[a][b] = fma(pr[a], pc[b], acc[a][b]);
-  }
+          for (int c2 = c + 1; c2 < NB; ++c2) a[c2] = fma(-v, Ds[c2][c], a[c2]);
+        }
 #pragma unroll
-  for (int a = 0; a < 4; ++a) {
-    int r = r0 + ty * 4 + a;
-    if (r >= rows_total) continue;
-#pragma unroll
-    for (int b = 0; b < 4; ++b) {
-      int c = c0 + tx * 4 + b;
-      if (c >= n0 || (r < n0 && c > r)) continue;
-      A[(size_t)r * n0 + c] -= acc[a][b];
+        for (int c = 0; c < NB; ++c)
+          if (c < nb) arow[c] = a[c];
+      }
     }
+    grid.sync();
+    // ---- phase 2 --------------------------------------------------------------------------------------
+    const int cols = n0 - j1;
+    if (cols > 0) {
+      const int ntc = (cols + 63) / 64, ntr = (below + 63) / 64;
+      // valid tiles only: for a row tile inside the square part, column tiles up to the diagonal
+      for (int t = blockIdx.x;; t += G) {
+        // map t to the t-th valid tile: rows tr < ntc are triangular (tr + 1 tiles), the rest are full
+        int tr, tc;
+        const int tri_tiles = ntc * (ntc + 1) / 2;
+        if (t < tri_tiles) {
+          tr = (int)((sqrt(8.0 * t + 1.0) - 1.0) * 0.5);
+          while (tr * (tr + 1) / 2 > t) --tr;
+          while ((tr + 1) * (tr + 2) / 2 <= t) ++tr;
+          tc = t - tr * (tr + 1) / 2;
+        } else {
+          int u = t - tri_tiles;
+          tr = ntc + u / ntc;
+          tc = u % ntc;
+        }
+        if (tr >= ntr) break;
+        const int r0 = j1 + tr * 64, c0 = j1 + tc * 64;
+        __syncthreads();
+        for (int e = tid; e < 64 * NB; e += 256) {
+          int row = e / NB, tt = e % NB;
+          int rr = r0 + row, cc = c0 + row;
+          Pr[tt][row] = (rr < rows_total && tt < nb) ? A[(size_t)rr * n0 + j0 + tt] : 0.0;
+          Pc[tt][row] = (cc < n0 && tt < nb) ? A[(size_t)cc * n0 + j0 + tt] : 0.0;
+        }
+        __syncthreads();
+        const int tx = tid % 16, ty = tid / 16;
+        double acc[4][4];
+#pragma unroll
+        for (int a_ = 0; a_ < 4; ++a_)
+#pragma unroll
+          for (int b_ = 0; b_ < 4; ++b_) acc[a_][b_] = 0.0;
+#pragma unroll 8
+        for (int tt = 0; tt < NB; ++tt) {
+          double pr[4], pc[4];
+#pragma unroll
+          for (int a_ = 0; a_ < 4; ++a_) { pr[a_] = Pr[tt][ty * 4 + a_]; pc[a_] = Pc[tt][tx * 4 + a_]; }
+#pragma unroll
+          for (int a_ = 0; a_ < 4; ++a_)
+#pragma unroll
+            for (int b_ = 0; b_ < 4; ++b_) acc[a_][b_] = fma(pr[a_], pc[b_], acc[a_][b_]);
+        }
+#pragma unroll
+        for (int a_ = 0; a_ < 4; ++a_) {
+          int r = r0 + ty * 4 + a_;
+          if (r >= rows_total) continue;
+#pragma unroll
+          for (int b_ = 0; b_ < 4; ++b_) {
+            int cidx = c0 + tx * 4 + b_;
+            if (cidx >= n0 || (r < n0 && cidx > r)) continue;
+            A[(size_t)r * n0 + cidx] -= acc[a_][b_];
+          }
+        }
+      }
+    }
+    grid.sync();
   }
 }
 
@@ -200,20 +240,21 @@ gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried) {
       head_carry_init_kernel<float><<<grid, 256, 0, c.st>>>((const float*)carried_src, n0, mode, A);
     GP_LAUNCH_CHECK();
   }
-  const int rows_total = n0 + n_carried;
-  for (int j0 = 0; j0 < n0; j0 += NB) {
-    int nb = n0 - j0 < NB ? n0 - j0 : NB;
-    int below = rows_total - (j0 + nb);
-    unsigned pg = below > 0 ? (unsigned)((below + 63) / 64) : 1u;
-    head_panel_kernel<<<pg, 64, 0, c.st>>>(A, n0, rows_total, j0, c.ctrl());
-    GP_LAUNCH_CHECK();
-    int cols = n0 - (j0 + nb);
-    if (cols > 0) {
-      dim3 ug((cols + 63) / 64, (below + 63) / 64);
-      head_update_kernel<<<ug, 256, 0, c.st>>>(A, n0, rows_total, j0, nb);
-      GP_LAUNCH_CHECK();
-    }
+  int rows_total = n0 + n_carried;
+  static int grid_ctas = 0;
+  if (grid_ctas == 0) {
+    int dev = 0, sms = 0, per_sm = 0;
+    GP_CUDA_OK(cudaGetDevice(&dev));
+    GP_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    GP_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, head_chol_kernel, 256, 0));
+    if (per_sm < 1) return GP_ERR_CUDA;
+    grid_ctas = sms;                                        // one CTA per SM: all co-resident
   }
+  int n0_arg = n0;
+  Control* ctrl = c.ctrl();
+  void* args[] = {(void*)&A, (void*)&n0_arg, (void*)&rows_total, (void*)&ctrl};
+  GP_CUDA_OK(cudaLaunchCooperativeKernel((const void*)head_chol_kernel, dim3(grid_ctas), dim3(256), args, 0, c.st));
+  GP_LAUNCH_CHECK();
   return GP_OK;
 }
 

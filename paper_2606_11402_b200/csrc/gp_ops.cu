@@ -12,16 +12,41 @@ enum { OPK_FORWARD = 0, OPK_INVERSE = 1, OPK_LOGDET = 2 };
 constexpr int kCondThreads = 128;
 
 // rec[i] = {x_i, vals_i or 0}
+// "value not produced yet" marker of the dataflow forward: an all-ones NaN.  The kernels never write it
+// (every NaN result is canonicalised to the quiet NaN 0x7fc0... first).
+template <typename T> struct Pending;
+template <> struct Pending<float> {
+  static __device__ __forceinline__ float make() { return __uint_as_float(0xffffffffu); }
+  static __device__ __forceinline__ bool is(float v) { return __float_as_uint(v) == 0xffffffffu; }
+  static __device__ __forceinline__ float load(const float* p) {
+    float v; asm volatile("ld.relaxed.gpu.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory"); return v;
+  }
+  static __device__ __forceinline__ void store(float* p, float v) {
+    asm volatile("st.relaxed.gpu.global.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory");
+  }
+};
+template <> struct Pending<double> {
+  static __device__ __forceinline__ double make() { return __longlong_as_double(-1LL); }
+  static __device__ __forceinline__ bool is(double v) { return __double_as_longlong(v) == -1LL; }
+  static __device__ __forceinline__ double load(const double* p) {
+    double v; asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory"); return v;
+  }
+  static __device__ __forceinline__ void store(double* p, double v) {
+    asm volatile("st.relaxed.gpu.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory");
+  }
+};
+
+// rec[i] = {x_i, vals_i | 0 | pending}
 template <typename T>
 __global__ void pack_kernel(const T* __restrict__ x, const T* __restrict__ vals, Rec<T>* __restrict__ rec,
-                            int64_t n, int d) {
+                            int64_t n, int d, int pending) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   Rec<T> r;
   r.x0 = x[i * d];
   r.x1 = d >= 2 ? x[i * d + 1] : T(0);
   r.x2 = d >= 3 ? x[i * d + 2] : T(0);
-  r.v = vals ? vals[i] : T(0);
+  r.v = vals ? vals[i] : (pending ? Pending<T>::make() : T(0));
   rec[i] = r;
 }
 
@@ -55,6 +80,74 @@ cond_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* 
     }
   }
   if (OP == OPK_LOGDET) block_atomic_add(ld, &ctrl->acc[0], red);
+}
+
+// ---- dataflow forward: ONE launch for all batches (Alg. 1 lines 2-8) --------------------
+// Every point i >= n0 is one thread.  CTAs take chunks of the graph order through a ticket, so a chunk with a
+// lower number has always started: its threads are resident and depend only on still earlier chunks, hence
+// polling cannot deadlock.  A thread first does everything that does not depend on values (indices,
+// coordinates, K, its factor, the weights w and s), then waits until the k neighbour values are no longer
+// "pending", and applies  v_i = w . v_c + sigma s xi_i.  In steady state the neighbours were produced long
+// ago and the first gather already returns them; only at the frontier (and in the small early batches, where
+// the per-batch latency chain of a launch-per-batch loop is what costs) does a thread poll.  The value word
+// is its own ready flag, so no fence or counter is involved.
+template <typename T, int K, int D, int KIND>
+__global__ void __launch_bounds__(kCondThreads)
+forward_flow_kernel(Rec<T>* rec, const int32_t* __restrict__ nbr, const T* __restrict__ xi, T* __restrict__ out,
+                    int64_t n0, int64_t n, KParams<T> kp, Control* ctrl) {
+  __shared__ unsigned long long s_chunk;
+  if (threadIdx.x == 0) s_chunk = atomicAdd(&ctrl->ticket, 1ULL);
+  __syncthreads();
+  const int64_t i = n0 + (int64_t)s_chunk * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int32_t* row = nbr + (i - n0) * K;
+  T w[K], vv[K];
+  Cond<T> c;
+  {
+    Rec<T> self = load_rec_l1(rec + i);
+    int32_t idx[K];
+    Rec<T> R[K];
+    load_row<K>(row, idx);
+#pragma unroll
+    for (int j = 0; j < K; ++j) R[j] = load_rec_l1(rec + idx[j]);
+#pragma unroll
+    for (int j = 0; j < K; ++j) vv[j] = R[j].v;
+    c = weights_reg<T, K, D, KIND>(R, self, kp, w);
+  }
+  bool missing = false;
+#pragma unroll
+  for (int j = 0; j < K; ++j) missing |= Pending<T>::is(vv[j]);
+  if (missing) {
+    int32_t idx[K];
+    load_row<K>(row, idx);
+    const long long t0 = clock64();
+    unsigned spins = 0;
+    while (true) {
+      missing = false;
+#pragma unroll
+      for (int j = 0; j < K; ++j) {
+        if (Pending<T>::is(vv[j])) {
+          vv[j] = Pending<T>::load(&rec[idx[j]].v);
+          missing |= Pending<T>::is(vv[j]);
+        }
+      }
+      if (!missing) break;
+      if (++spins > 8) __nanosleep(spins > 64 ? 256 : 32);
+      if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) {   // watchdog (about 4 s): a bug, never expected
+        atomicAdd(&ctrl->timeout, 1ULL);
+        c.ok = false;
+        break;
+      }
+    }
+  }
+  T m = T(0);
+#pragma unroll
+  for (int j = 0; j < K; ++j) m = Math<T>::fma(w[j], vv[j], m);
+  T v = Math<T>::fma(kp.sigma * c.s, xi[i], m);
+  if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
+  if (!c.ok || v != v) v = quiet_nan<T>();
+  out[i] = v;
+  Pending<T>::store(&rec[i].v, v);
 }
 
 template <typename T, int OP>
@@ -174,10 +267,10 @@ static gp_status launch_range(const OpCtx& c, bool spec, const T* vals, const T*
 }
 
 template <typename T>
-static gp_status pack(const OpCtx& c, const T* vals) {
+static gp_status pack(const OpCtx& c, const T* vals, bool pending = false) {
   int64_t n = c.g->n;
   unsigned grid = (unsigned)((n + 255) / 256);
-  pack_kernel<T><<<grid, 256, 0, c.st>>>((const T*)c.g->x, vals, (Rec<T>*)c.rec(), n, c.g->d);
+  pack_kernel<T><<<grid, 256, 0, c.st>>>((const T*)c.g->x, vals, (Rec<T>*)c.rec(), n, c.g->d, pending ? 1 : 0);
   GP_LAUNCH_CHECK();
   return GP_OK;
 }
@@ -192,13 +285,44 @@ __global__ void finalize_logdet_kernel(const Control* ctrl, double* logdet, doub
   }
 }
 
+template <typename T, int K, int D>
+static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
+  int64_t cnt = c.g->n - c.g->n0;
+  if (cnt <= 0) return GP_OK;
+  unsigned grid = (unsigned)((cnt + kCondThreads - 1) / kCondThreads);
+  KParams<T> kp = make_kparams<T>(*c.kern);
+  Rec<T>* rec = (Rec<T>*)c.rec();
+  switch (c.kern->kind) {
+    case GP_KERNEL_SE:
+      forward_flow_kernel<T, K, D, GP_KERNEL_SE><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, c.g->n, kp, c.ctrl());
+      break;
+    case GP_KERNEL_MATERN32:
+      forward_flow_kernel<T, K, D, GP_KERNEL_MATERN32><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, c.g->n, kp, c.ctrl());
+      break;
+    default:
+      forward_flow_kernel<T, K, D, GP_KERNEL_EXP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, c.g->n, kp, c.ctrl());
+      break;
+  }
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
 template <typename T>
 static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
   bool spec = use_spec(c);
+  bool flow = spec && !(c.g->flags & GP_FLAG_PER_BATCH_LAUNCH);
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
-  if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr));
+  if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr, flow));
   GP_OK_OR_RETURN(head_factor(c, nullptr, 0));
   GP_OK_OR_RETURN(head_forward(c, xi, v, c.rec(), spec));
+  if (flow) {
+#define X(TT, K, D) \
+    if constexpr (std::is_same<TT, T>::value) {                    \
+      if (c.g->k == K && c.g->d == D) return launch_flow<T, K, D>(c, xi, v); \
+    }
+    GP_SPEC_TABLE(X)
+#undef X
+  }
   const int64_t* off = c.g->batch_off;
   for (int b = 0; b < c.g->n_batches; ++b)
     GP_OK_OR_RETURN((launch_range<T, OPK_FORWARD>(c, spec, v, xi, v, off[b], off[b + 1])));

@@ -208,3 +208,32 @@ def test_argument_errors(gp, orc):
     G2 = gp.Graph(x=G.x, nbr=G.nbr, batch_off=bad, n0=G.n0)
     with pytest.raises(gp.GraphGPError):
         gp.gp_forward(G2, gp.Kernel("se", 1.0, 0.1, 1e-6), xi)
+
+
+@pytest.mark.parametrize("cid,n,dtype", [(1, 4096, "f64"), (2, 50000, "f32"), (3, 30011, "f32")])
+def test_dataflow_forward_equals_per_batch_forward(gp, orc, cid, n, dtype):
+    """The single-launch dataflow forward and the literal loop over batches of Alg. 1 apply the
+    same weights to the same neighbour values: they agree to rounding (the weights are reached by a different
+    substitution order), and both match the oracle."""
+    import torch
+    cfg = W.CONFIGS[cid]
+    g = oracle_graph(orc, cid, n, dtype)
+    tdt = torch.float64 if dtype == "f64" else torch.float32
+    xi_h = W.make_noise(cid, n, dtype, "xi")
+    xi = torch.as_tensor(xi_h, device="cuda").to(tdt)
+    K = gp.Kernel(**kern_of(cfg))
+    outs = []
+    for flags in (0, gp.GP_FLAG_PER_BATCH_LAUNCH):
+        G = to_dev(gp, g, dtype, flags)
+        for _ in range(3):                       # repeated calls reuse the workspace: pending markers are reset
+            v = gp.gp_forward(G, K, xi)
+        assert gp.check_errors(G.workspace(gp.GP_OP_FORWARD)) == 0
+        outs.append(v.cpu().numpy().astype(np.float64))
+    v_ref = orc.forward(g.x, orc.Kernel(**kern_of(cfg)), xi_h.astype(np.float64), n0=g.n0, k=g.k, nbr=g.nbr,
+                        batch_off=g.batch_off)
+    tol = F64_TOL if dtype == "f64" else F32_V_TOL
+    scale = np.abs(v_ref).max() if dtype == "f64" else v_ref.std()
+    assert np.isfinite(outs[0]).all()
+    assert np.abs(outs[0] - outs[1]).max() / scale <= tol
+    assert np.abs(outs[0] - v_ref).max() / scale <= tol
+    assert np.abs(outs[1] - v_ref).max() / scale <= tol
