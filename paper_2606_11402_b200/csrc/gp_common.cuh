@@ -43,6 +43,7 @@ struct KParams {
   T sigma;
   T diag;    // 1 + eps
   T inv_ell;
+  T sq;      // sqrt(qscale): the packed fp32 path scales the centred coordinates once instead of every q
 };
 
 template <typename T> __host__ inline KParams<T> make_kparams(const gp_kernel& k);
@@ -57,6 +58,7 @@ template <> __host__ inline KParams<float> make_kparams<float>(const gp_kernel& 
   }
   p.qscale = (float)s; p.eps = (float)k.jitter; p.sigma = (float)k.sigma; p.diag = (float)(1.0 + k.jitter);
   p.inv_ell = (float)(1.0 / k.ell);
+  p.sq = (float)sqrt(s);
   return p;
 }
 template <> __host__ inline KParams<double> make_kparams<double>(const gp_kernel& k) {
@@ -68,6 +70,7 @@ template <> __host__ inline KParams<double> make_kparams<double>(const gp_kernel
     default: s = 1.0 / (k.ell * k.ell); break;
   }
   p.qscale = s; p.eps = k.jitter; p.sigma = k.sigma; p.diag = 1.0 + k.jitter; p.inv_ell = 1.0 / k.ell;
+  p.sq = sqrt(s);
   return p;
 }
 

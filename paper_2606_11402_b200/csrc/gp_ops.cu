@@ -4,7 +4,7 @@
 //   logdet   PAPER.md:9:  sum_i log s_i^2, fp64 accumulation
 #include <type_traits>
 
-#include "gp_cond.cuh"
+#include "gp_cond_pk.cuh"
 
 namespace gp {
 
@@ -63,7 +63,11 @@ cond_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* 
   double ld = 0.0;
   if (i < end) {
     Rec<T> self = load_rec<false>(rec + i);
-    Cond<T> c = condition_reg<T, K, D, KIND, false>(rec, nbr + (i - n0) * K, self, kp);
+    Cond<T> c;
+    if constexpr (std::is_same<T, float>::value && K % 2 == 0)
+      c = condition_pk<K, D, KIND, false>(rec, nbr + (i - n0) * K, self, kp);
+    else
+      c = condition_reg<T, K, D, KIND, false>(rec, nbr + (i - n0) * K, self, kp);
     T ss = kp.sigma * c.s;
     if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
     if (OP == OPK_FORWARD) {
@@ -112,7 +116,8 @@ forward_flow_kernel(Rec<T>* rec, const int32_t* __restrict__ nbr, const T* __res
     for (int j = 0; j < K; ++j) R[j] = load_rec_l1(rec + idx[j]);
 #pragma unroll
     for (int j = 0; j < K; ++j) vv[j] = R[j].v;
-    c = weights_reg<T, K, D, KIND>(R, self, kp, w);
+    if constexpr (std::is_same<T, float>::value && K % 2 == 0) c = weights_pk<K, D, KIND>(R, self, kp, w);
+    else c = weights_reg<T, K, D, KIND>(R, self, kp, w);
   }
   bool missing = false;
 #pragma unroll
