@@ -9,6 +9,33 @@ namespace gp {
 static std::atomic<long long> g_launches{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+gp_status side_stream(SideStream** out) {
+  static SideStream per_dev[64];
+  int dev = 0;
+  GP_CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return GP_ERR_CUDA;
+  SideStream& s = per_dev[dev];
+  if (!s.stream) {
+    int lo = 0, hi = 0;
+    GP_CUDA_OK(cudaDeviceGetStreamPriorityRange(&lo, &hi));
+    GP_CUDA_OK(cudaStreamCreateWithPriority(&s.stream, cudaStreamNonBlocking, hi));
+    GP_CUDA_OK(cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming));
+    GP_CUDA_OK(cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming));
+  }
+  *out = &s;
+  return GP_OK;
+}
+gp_status side_fork(const SideStream* s, cudaStream_t main) {
+  GP_CUDA_OK(cudaEventRecord(s->fork, main));
+  GP_CUDA_OK(cudaStreamWaitEvent(s->stream, s->fork, 0));
+  return GP_OK;
+}
+gp_status side_join(const SideStream* s, cudaStream_t main) {
+  GP_CUDA_OK(cudaEventRecord(s->join, s->stream));
+  GP_CUDA_OK(cudaStreamWaitEvent(main, s->join, 0));
+  return GP_OK;
+}
+
 static gp_status validate(const gp_graph* g, const gp_kernel* kern) {
   if (!g || !kern) return GP_ERR_INVALID_ARG;
   if (g->n <= 0 || g->n0 < 0 || g->n0 > g->n) return GP_ERR_INVALID_ARG;

@@ -208,6 +208,18 @@ struct OpCtx {
   void* gbar() const { return ws + lay.g_off; }
 };
 
+// Fork/join helper: the dense head is independent of the bulk conditioning in gp_inverse / gp_logdet / gp_vjp,
+// so it runs on a library-internal high-priority stream between a fork event (recorded on the caller's
+// stream) and a join event (waited on by the caller's stream).  One stream and two events per device are
+// created lazily on first use and never destroyed; everything stays ordered with respect to the caller's stream.
+struct SideStream {
+  cudaStream_t stream = nullptr;
+  cudaEvent_t fork = nullptr, join = nullptr;
+};
+gp_status side_stream(SideStream** out);
+gp_status side_fork(const SideStream* s, cudaStream_t main);   // side waits for everything queued on main so far
+gp_status side_join(const SideStream* s, cudaStream_t main);   // main waits for everything queued on side so far
+
 // ---- entry points implemented across the .cu files ------------------------------------------------
 // dense head (gp_head.cu)
 gp_status head_factor(const OpCtx& c, const void* carried_src /*dtype [n0] or null*/, int n_carried);

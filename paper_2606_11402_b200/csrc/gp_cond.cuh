@@ -44,6 +44,13 @@ __device__ __forceinline__ Rec<double> load_rec_l1(const Rec<double>* p) {
   Rec<double> r; r.x0 = a; r.x1 = b; r.x2 = c; r.v = d; return r;
 }
 
+__device__ __forceinline__ float load_val_l1(const float* p) {
+  float v; asm volatile("ld.global.ca.f32 %0, [%1];" : "=f"(v) : "l"(p)); return v;
+}
+__device__ __forceinline__ double load_val_l1(const double* p) {
+  double v; asm volatile("ld.global.ca.f64 %0, [%1];" : "=d"(v) : "l"(p)); return v;
+}
+
 template <typename T, int D> __device__ __forceinline__ T pair_q(const Rec<T>& a, const Rec<T>& b, T qscale) {
   T dx = a.x0 - b.x0;
   T d2 = dx * dx;

@@ -83,8 +83,7 @@ template <int J> struct DiagStep {
   static __device__ __forceinline__ void run(double (&a)[NB], int lane, double* invd, bool& bad) {
     double piv = shfl_d(a[J], J);
     bad |= !(piv > 0.0);
-    double inv = rsqrt(piv);
-    inv = inv * fma(-0.5 * piv * inv, inv, 1.5);     // one Newton step: full double accuracy
+    double inv = rsqrt(piv);                          // CUDA's double rsqrt: 1 ulp
     double lj = a[J] * inv;                           // lane J: sqrt(piv); lanes > J: L[lane][J]
     a[J] = lj;
     if (lane == J) invd[J] = inv;

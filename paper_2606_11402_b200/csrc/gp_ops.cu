@@ -10,6 +10,12 @@ namespace gp {
 
 enum { OPK_FORWARD = 0, OPK_INVERSE = 1, OPK_LOGDET = 2 };
 constexpr int kCondThreads = 128;
+#ifndef GP_COND_MIN_CTAS
+#define GP_COND_MIN_CTAS 3
+#endif
+#ifndef GP_FLOW_MIN_CTAS
+#define GP_FLOW_MIN_CTAS 3
+#endif
 
 // rec[i] = {x_i, vals_i or 0}
 // "value not produced yet" marker of the dataflow forward: an all-ones NaN.  The kernels never write it
@@ -55,7 +61,7 @@ template <> __device__ __forceinline__ float quiet_nan<float>() { return __int_a
 template <> __device__ __forceinline__ double quiet_nan<double>() { return __longlong_as_double(0x7ff8000000000000LL); }
 
 template <typename T, int K, int D, int KIND, int OP>
-__global__ void __launch_bounds__(kCondThreads)
+__global__ void __launch_bounds__(kCondThreads, GP_COND_MIN_CTAS)
 cond_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* __restrict__ in,
             T* __restrict__ out, int64_t start, int64_t end, int64_t n0, KParams<T> kp, Control* ctrl) {
   __shared__ double red[32];
@@ -96,7 +102,7 @@ cond_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* 
 // the per-batch latency chain of a launch-per-batch loop is what costs) does a thread poll.  The value word
 // is its own ready flag, so no fence or counter is involved.
 template <typename T, int K, int D, int KIND>
-__global__ void __launch_bounds__(kCondThreads)
+__global__ void __launch_bounds__(kCondThreads, GP_FLOW_MIN_CTAS)
 forward_flow_kernel(Rec<T>* rec, const int32_t* __restrict__ nbr, const T* __restrict__ xi, T* __restrict__ out,
                     int64_t n0, int64_t n, KParams<T> kp, Control* ctrl) {
   __shared__ unsigned long long s_chunk;
@@ -105,7 +111,7 @@ forward_flow_kernel(Rec<T>* rec, const int32_t* __restrict__ nbr, const T* __res
   const int64_t i = n0 + (int64_t)s_chunk * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int32_t* row = nbr + (i - n0) * K;
-  T w[K], vv[K];
+  T w[K];
   Cond<T> c;
   {
     Rec<T> self = load_rec_l1(rec + i);
@@ -114,34 +120,36 @@ forward_flow_kernel(Rec<T>* rec, const int32_t* __restrict__ nbr, const T* __res
     load_row<K>(row, idx);
 #pragma unroll
     for (int j = 0; j < K; ++j) R[j] = load_rec_l1(rec + idx[j]);
-#pragma unroll
-    for (int j = 0; j < K; ++j) vv[j] = R[j].v;
     if constexpr (std::is_same<T, float>::value && K % 2 == 0) c = weights_pk<K, D, KIND>(R, self, kp, w);
     else c = weights_reg<T, K, D, KIND>(R, self, kp, w);
   }
-  bool missing = false;
-#pragma unroll
-  for (int j = 0; j < K; ++j) missing |= Pending<T>::is(vv[j]);
-  if (missing) {
+  // values: read again now (the lines are in L1 from the gather above; a stale "pending" is re-read from L2)
+  T vv[K];
+  {
     int32_t idx[K];
     load_row<K>(row, idx);
-    const long long t0 = clock64();
-    unsigned spins = 0;
-    while (true) {
-      missing = false;
+    bool missing = false;
 #pragma unroll
-      for (int j = 0; j < K; ++j) {
-        if (Pending<T>::is(vv[j])) {
-          vv[j] = Pending<T>::load(&rec[idx[j]].v);
-          missing |= Pending<T>::is(vv[j]);
+    for (int j = 0; j < K; ++j) { vv[j] = load_val_l1(&rec[idx[j]].v); missing |= Pending<T>::is(vv[j]); }
+    if (missing) {
+      const long long t0 = clock64();
+      unsigned spins = 0;
+      while (true) {
+        missing = false;
+#pragma unroll
+        for (int j = 0; j < K; ++j) {
+          if (Pending<T>::is(vv[j])) {
+            vv[j] = Pending<T>::load(&rec[idx[j]].v);
+            missing |= Pending<T>::is(vv[j]);
+          }
         }
-      }
-      if (!missing) break;
-      if (++spins > 8) __nanosleep(spins > 64 ? 256 : 32);
-      if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) {   // watchdog (about 4 s): a bug, never expected
-        atomicAdd(&ctrl->timeout, 1ULL);
-        c.ok = false;
-        break;
+        if (!missing) break;
+        if (++spins > 8) __nanosleep(spins > 64 ? 256 : 32);
+        if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) {   // watchdog (about 4 s): a bug, never expected
+          atomicAdd(&ctrl->timeout, 1ULL);
+          c.ok = false;
+          break;
+        }
       }
     }
   }
@@ -338,21 +346,34 @@ template <typename T>
 static gp_status inverse_t(const OpCtx& c, const T* v, T* xi) {
   bool spec = use_spec(c);
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
+  // the head (xi[0:n0]) and the bulk (xi[n0:n]) are independent: head on the side stream, submitted first
+  SideStream* side = nullptr;
+  GP_OK_OR_RETURN(side_stream(&side));
+  GP_OK_OR_RETURN(side_fork(side, c.st));
+  OpCtx hc = c;
+  hc.st = side->stream;
+  GP_OK_OR_RETURN(head_factor(hc, v, 1));
+  GP_OK_OR_RETURN(head_inverse_out(hc, xi));
   if (spec) GP_OK_OR_RETURN(pack<T>(c, v));
-  GP_OK_OR_RETURN(head_factor(c, v, 1));
-  GP_OK_OR_RETURN(head_inverse_out(c, xi));
-  return launch_range<T, OPK_INVERSE>(c, spec, v, v, xi, c.g->n0, c.g->n);
+  GP_OK_OR_RETURN((launch_range<T, OPK_INVERSE>(c, spec, v, v, xi, c.g->n0, c.g->n)));
+  return side_join(side, c.st);
 }
 
 template <typename T>
 static gp_status logdet_t(const OpCtx& c, double* logdet, double* grad) {
   bool spec = use_spec(c);
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
+  SideStream* side = nullptr;
+  GP_OK_OR_RETURN(side_stream(&side));
+  GP_OK_OR_RETURN(side_fork(side, c.st));
+  OpCtx hc = c;
+  hc.st = side->stream;
+  GP_OK_OR_RETURN(head_factor(hc, nullptr, grad ? 2 * (int)c.g->n0 : 0));
+  GP_OK_OR_RETURN(head_logdet(hc, &c.ctrl()->acc[0], grad ? &c.ctrl()->acc[2] : nullptr));
   if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr));
-  GP_OK_OR_RETURN(head_factor(c, nullptr, grad ? 2 * (int)c.g->n0 : 0));
-  GP_OK_OR_RETURN(head_logdet(c, &c.ctrl()->acc[0], grad ? &c.ctrl()->acc[2] : nullptr));
   GP_OK_OR_RETURN((launch_range<T, OPK_LOGDET>(c, spec, nullptr, nullptr, nullptr, c.g->n0, c.g->n)));
   if (grad) GP_OK_OR_RETURN(run_logdet_grad(c));
+  GP_OK_OR_RETURN(side_join(side, c.st));
   finalize_logdet_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), logdet, grad, 2.0 * (double)c.g->n / c.kern->sigma,
                                              1.0 / c.kern->ell);
   GP_LAUNCH_CHECK();

@@ -283,14 +283,21 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
   T* gbar = (T*)c.gbar();
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
   GP_CUDA_OK(cudaMemcpyAsync(gbar, vbar, (size_t)n * sizeof(T), cudaMemcpyDeviceToDevice, c.st));
+  // the head factorisation does not depend on the cotangents: side stream, overlapped with the reverse sweep
+  SideStream* side = nullptr;
+  GP_OK_OR_RETURN(side_stream(&side));
+  GP_OK_OR_RETURN(side_fork(side, c.st));
+  if (n0 > 0) {
+    OpCtx hc = c;
+    hc.st = side->stream;
+    GP_OK_OR_RETURN(head_factor(hc, nullptr, 2 * (int)n0));
+  }
   if (spec) GP_OK_OR_RETURN(grad_pack<T>(c, v));
   const int64_t* off = c.g->batch_off;
   for (int b = c.g->n_batches - 1; b >= 0; --b)
     GP_OK_OR_RETURN((launch_grad_range<T, GRAD_VJP>(c, spec, v, xi, gbar, xibar, off[b], off[b + 1])));
-  if (n0 > 0) {
-    GP_OK_OR_RETURN(head_factor(c, nullptr, 2 * (int)n0));
-    GP_OK_OR_RETURN(head_vjp(c, xi, gbar, xibar, &c.ctrl()->acc[3]));
-  }
+  GP_OK_OR_RETURN(side_join(side, c.st));
+  if (n0 > 0) GP_OK_OR_RETURN(head_vjp(c, xi, gbar, xibar, &c.ctrl()->acc[3]));
   finalize_grad_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), 3, 4, 1.0 / c.kern->ell, thetabar);
   GP_LAUNCH_CHECK();
   return GP_OK;
