@@ -222,7 +222,9 @@ gp_status side_join(const SideStream* s, cudaStream_t main);   // main waits for
 
 // ---- entry points implemented across the .cu files ------------------------------------------------
 // dense head (gp_head.cu)
-gp_status head_factor(const OpCtx& c, const void* carried_src /*dtype [n0] or null*/, int n_carried);
+// overlapped: the factorisation runs beside the bulk kernel on the side stream -> use few CTAs so that most
+// SMs keep their full bulk occupancy; otherwise (forward: the head is on the critical path) one CTA per SM.
+gp_status head_factor(const OpCtx& c, const void* carried_src /*dtype [n0] or null*/, int n_carried, bool overlapped = false);
 gp_status head_forward(const OpCtx& c, const void* xi, void* v, void* rec, bool rec_is_packed);
 gp_status head_inverse_out(const OpCtx& c, void* xi);
 gp_status head_logdet(const OpCtx& c, double* acc /*device: acc[0] += logdet head*/,

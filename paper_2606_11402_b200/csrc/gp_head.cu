@@ -212,7 +212,7 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
   }
 }
 
-gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried) {
+gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried, bool overlapped) {
   const int n0 = (int)c.g->n0;
   if (n0 <= 0) return GP_OK;
   double* A = c.head();
@@ -252,7 +252,12 @@ gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried) {
   int n0_arg = n0;
   Control* ctrl = c.ctrl();
   void* args[] = {(void*)&A, (void*)&n0_arg, (void*)&rows_total, (void*)&ctrl};
-  GP_CUDA_OK(cudaLaunchCooperativeKernel((const void*)head_chol_kernel, dim3(grid_ctas), dim3(256), args, 0, c.st));
+  int ctas = grid_ctas;
+  if (overlapped) {                                         // a quarter of the SMs; more when many rows are carried
+    ctas = n_carried > n0 ? grid_ctas / 2 : grid_ctas / 4;
+    if (ctas < 1) ctas = 1;
+  }
+  GP_CUDA_OK(cudaLaunchCooperativeKernel((const void*)head_chol_kernel, dim3(ctas), dim3(256), args, 0, c.st));
   GP_LAUNCH_CHECK();
   return GP_OK;
 }

@@ -325,8 +325,17 @@ static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
   bool spec = use_spec(c);
   bool flow = spec && !(c.g->flags & GP_FLAG_PER_BATCH_LAUNCH);
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
-  if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr, flow));
+  // the head is on the critical path (every batch depends on it); packing the records is not: side stream
+  SideStream* side = nullptr;
+  GP_OK_OR_RETURN(side_stream(&side));
+  if (spec) {
+    GP_OK_OR_RETURN(side_fork(side, c.st));
+    OpCtx pc = c;
+    pc.st = side->stream;
+    GP_OK_OR_RETURN(pack<T>(pc, nullptr, flow));
+  }
   GP_OK_OR_RETURN(head_factor(c, nullptr, 0));
+  if (spec) GP_OK_OR_RETURN(side_join(side, c.st));
   GP_OK_OR_RETURN(head_forward(c, xi, v, c.rec(), spec));
   if (flow) {
 #define X(TT, K, D) \
@@ -352,7 +361,7 @@ static gp_status inverse_t(const OpCtx& c, const T* v, T* xi) {
   GP_OK_OR_RETURN(side_fork(side, c.st));
   OpCtx hc = c;
   hc.st = side->stream;
-  GP_OK_OR_RETURN(head_factor(hc, v, 1));
+  GP_OK_OR_RETURN(head_factor(hc, v, 1, true));
   GP_OK_OR_RETURN(head_inverse_out(hc, xi));
   if (spec) GP_OK_OR_RETURN(pack<T>(c, v));
   GP_OK_OR_RETURN((launch_range<T, OPK_INVERSE>(c, spec, v, v, xi, c.g->n0, c.g->n)));
@@ -368,7 +377,7 @@ static gp_status logdet_t(const OpCtx& c, double* logdet, double* grad) {
   GP_OK_OR_RETURN(side_fork(side, c.st));
   OpCtx hc = c;
   hc.st = side->stream;
-  GP_OK_OR_RETURN(head_factor(hc, nullptr, grad ? 2 * (int)c.g->n0 : 0));
+  GP_OK_OR_RETURN(head_factor(hc, nullptr, grad ? 2 * (int)c.g->n0 : 0, true));
   GP_OK_OR_RETURN(head_logdet(hc, &c.ctrl()->acc[0], grad ? &c.ctrl()->acc[2] : nullptr));
   if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr));
   GP_OK_OR_RETURN((launch_range<T, OPK_LOGDET>(c, spec, nullptr, nullptr, nullptr, c.g->n0, c.g->n)));

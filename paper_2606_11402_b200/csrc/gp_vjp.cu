@@ -290,7 +290,7 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
   if (n0 > 0) {
     OpCtx hc = c;
     hc.st = side->stream;
-    GP_OK_OR_RETURN(head_factor(hc, nullptr, 2 * (int)n0));
+    GP_OK_OR_RETURN(head_factor(hc, nullptr, 2 * (int)n0, true));
   }
   if (spec) GP_OK_OR_RETURN(grad_pack<T>(c, v));
   const int64_t* off = c.g->batch_off;
