@@ -425,7 +425,7 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
   GP_CUDA_OK(cudaMemsetAsync(depth_tree, 0, (size_t)n * 4, st));
   int64_t max_depth = 0;
   if (n > n0) {
-    unsigned long long* flag = &ctrl->pad0;
+    unsigned long long* flag = &ctrl->done;   // builder reuses this slot as its "changed" flag
     for (int guard = 0; guard < (1 << 22); ++guard) {
       for (int r = 0; r < 3; ++r) {
         depth_sweep_kernel<<<nblk(n - n0), 256, 0, st>>>(nbr_tree, n, n0, k, depth_tree, flag);

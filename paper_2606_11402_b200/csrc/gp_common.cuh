@@ -20,7 +20,7 @@ struct Control {
   unsigned long long n_bad;    // points whose conditional was not positive definite
   unsigned long long ticket;   // dataflow forward: next chunk to hand out
   unsigned long long timeout;  // dataflow watchdog fired (a bug, never expected)
-  unsigned long long pad0;
+  unsigned long long done;     // dataflow VJP: points whose cotangent scatter is complete (reverse order)
   double acc[8];               // [0] logdet  [1] dlogdet/dsigma  [2] dlogdet/dell  [3] theta_bar sigma  [4] theta_bar ell
   double build_ms[4];          // graph builder stage times
   unsigned long long pad[4];

@@ -19,12 +19,17 @@
 // batch has scattered into it, and points of one batch never touch each other's cotangent.
 #include <type_traits>
 
-#include "gp_cond.cuh"
+#include <vector>
+
+#include "gp_grad_pk.cuh"
 
 namespace gp {
 
 enum { GRAD_VJP = 0, GRAD_LOGDET = 1 };
 constexpr int kGradThreads = 128;
+#ifndef GP_GRAD_MIN_CTAS
+#define GP_GRAD_MIN_CTAS 2
+#endif
 
 template <typename T> __device__ __forceinline__ T qnan();
 template <> __device__ __forceinline__ float qnan<float>() { return __int_as_float(0x7fc00000); }
@@ -117,6 +122,147 @@ grad_kernel(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, con
   }
   if (MODE == GRAD_VJP) block_atomic_add(acc_sigma, &ctrl->acc[3], red);
   block_atomic_add(acc_ell, &ctrl->acc[MODE == GRAD_VJP ? 4 : 2], red);
+}
+
+// ---- packed fp32 gradient kernels ----------------------------------------------------------------------------
+// Everything that does not depend on the incoming cotangent (weights w, s, and the two scalars
+//   A_i = y[0:k].alpha + sigma xi_i (y.u) / (2 s),   B_i = s xi_i      (ell_bar += g A_i, sigma_bar += g B_i))
+// is computed first; only then does the point need its total cotangent g.
+template <int K, int D, int KIND>
+__device__ __forceinline__ bool grad_geometry_pk(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ row,
+                                                 const Rec<float>& self, const KParams<float>& kp, const DqStore<K>& dq,
+                                                 f2 (&W)[K / 2], f2 (&AL)[K / 2], float& s) {
+  f2 P[pk_pairs(K)];
+  {
+    int32_t idx[K];
+    Rec<float> R[K];
+    gather_reg<float, K, false>(rec, row, idx, R);
+    PkCoords<K> X;
+    centre_pk<K, D>(R, self, kp.sq, X);
+    float vals[K];
+#pragma unroll
+    for (int j = 0; j < K; ++j) vals[j] = R[j].v;
+    build_joint_grad_pk<K, D, KIND>(X, vals, kp, P, dq);
+  }
+  bool ok = factor_joint_pk<K, true>(P, kp.diag);
+  s = Math<float>::sqrt(P[pk(K / 2, K)].x);
+  backsub2_pk<K>(P, W, AL);
+  return ok;
+}
+
+template <int K>
+__device__ __forceinline__ DqStore<K> dq_store_of(void* smem) {
+  DqStore<K> dq;
+  dq.p2 = reinterpret_cast<float2*>(smem) + threadIdx.x;
+  dq.p1 = reinterpret_cast<float*>(reinterpret_cast<float2*>(smem) + (size_t)dq_full_total(K) * blockDim.x) + threadIdx.x;
+  dq.stride = blockDim.x;
+  return dq;
+}
+
+// gradient of the log-determinant, conditioning part: every point at once
+template <int K, int D, int KIND>
+__global__ void __launch_bounds__(kGradThreads, GP_GRAD_MIN_CTAS)
+logdet_grad_pk_kernel(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ nbr, int64_t start, int64_t end,
+                      int64_t n0, KParams<float> kp, Control* ctrl) {
+  extern __shared__ float4 dq_raw[];
+  __shared__ double red[32];
+  int64_t i = start + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  double acc_ell = 0.0;
+  if (i < end) {
+    DqStore<K> dq = dq_store_of<K>(dq_raw);
+    Rec<float> self = load_rec<false>(rec + i);
+    f2 W[K / 2], AL[K / 2];
+    float s;
+    bool ok = grad_geometry_pk<K, D, KIND>(rec, nbr + (i - n0) * K, self, kp, dq, W, AL, s);
+#pragma unroll
+    for (int rp = 0; rp < K / 2; ++rp) AL[rp] = make_float2(0.0f, 0.0f);
+    float half_yu = grad_sweep_pk<K>(W, AL, 1.0f, dq);
+    if (!ok) atomicAdd(&ctrl->n_bad, 1ULL);
+    else acc_ell = (double)(2.0f * half_yu / (s * s));
+  }
+  block_atomic_add(acc_ell, &ctrl->acc[2], red);
+}
+
+// VJP of the forward pass in ONE launch, batches in reverse order.  CTAs take batch-aligned chunks through a
+// ticket (last batch first).  A chunk of batch b may read its cotangents once every point of every later batch
+// has scattered: ctrl->done counts finished points, so the test is done >= n - batch_off[b + 1].  Lower tickets
+// have always started and never wait on higher ones, so polling cannot deadlock.
+template <int K, int D, int KIND>
+__global__ void __launch_bounds__(kGradThreads, GP_GRAD_MIN_CTAS)
+vjp_flow_kernel(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ nbr, const float* __restrict__ xi,
+                float* gbar, float* __restrict__ xibar, const int64_t* __restrict__ boff,
+                const int64_t* __restrict__ cstart, int L, int64_t n0, int64_t n, KParams<float> kp, Control* ctrl) {
+  extern __shared__ float4 dq_raw[];
+  __shared__ double red[32];
+  __shared__ long long s_info[3];
+  if (threadIdx.x == 0) {
+    long long t = (long long)atomicAdd(&ctrl->ticket, 1ULL);
+    int lo = 0, hi = L - 1;                      // largest rb with cstart[rb] <= t
+    while (lo < hi) {
+      int mid = (lo + hi + 1) >> 1;
+      if (cstart[mid] <= t) lo = mid; else hi = mid - 1;
+    }
+    int b = L - 1 - lo;
+    s_info[0] = boff[b] + (t - cstart[lo]) * (long long)blockDim.x;
+    s_info[1] = boff[b + 1];
+    s_info[2] = n - boff[b + 1];
+  }
+  __syncthreads();
+  const int64_t i = s_info[0] + threadIdx.x;
+  const int64_t end = s_info[1];
+  const bool active = i < end;
+  const int32_t* row = nbr + (i - n0) * K;
+  f2 W[K / 2];
+  float s = 0.0f, Ai = 0.0f, Bi = 0.0f;
+  bool ok = true;
+  if (active) {
+    DqStore<K> dq = dq_store_of<K>(dq_raw);
+    Rec<float> self = load_rec<false>(rec + i);
+    f2 AL[K / 2];
+    ok = grad_geometry_pk<K, D, KIND>(rec, row, self, kp, dq, W, AL, s);
+    const float xi_i = xi[i];
+    Ai = grad_sweep_pk<K>(W, AL, kp.sigma * xi_i / s, dq);
+    Bi = s * xi_i;
+  }
+  if (threadIdx.x == 0) {
+    const unsigned long long need = (unsigned long long)s_info[2];
+    const long long t0 = clock64();
+    unsigned spins = 0;
+    while (true) {
+      unsigned long long d;
+      asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(d) : "l"(&ctrl->done) : "memory");
+      if (d >= need) break;
+      if (++spins > 4) __nanosleep(64);
+      if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) { atomicAdd(&ctrl->timeout, 1ULL); break; }
+    }
+  }
+  __syncthreads();
+  double acc_sigma = 0.0, acc_ell = 0.0;
+  if (active) {
+    const float g = __ldcg(gbar + i);
+    float out = kp.sigma * g * s;
+    if (!ok) { atomicAdd(&ctrl->n_bad, 1ULL); out = qnan<float>(); }
+    xibar[i] = out;
+    if (ok) {
+      int32_t idx[K];
+      load_row<K>(row, idx);
+#pragma unroll
+      for (int rp = 0; rp < K / 2; ++rp) {
+        atomicAdd(gbar + idx[2 * rp], g * W[rp].x);
+        atomicAdd(gbar + idx[2 * rp + 1], g * W[rp].y);
+      }
+      acc_sigma = (double)(g * Bi);
+      acc_ell = (double)(g * Ai);
+    }
+  }
+  __threadfence();
+  block_atomic_add(acc_sigma, &ctrl->acc[3], red);
+  block_atomic_add(acc_ell, &ctrl->acc[4], red);
+  if (threadIdx.x == 0) {
+    long long cnt = end - s_info[0];
+    if (cnt > (long long)blockDim.x) cnt = blockDim.x;
+    atomicAdd(&ctrl->done, (unsigned long long)cnt);
+  }
 }
 
 // ---- generic gradient kernel: triangle in shared memory, any k <= 64, d <= 4 -----------------------------
@@ -276,6 +422,73 @@ __global__ void finalize_grad_kernel(const Control* ctrl, int slot_sigma, int sl
   }
 }
 
+// ---- packed fp32 host side ------------------------------------------------------------------------------------
+template <typename KernelT> static gp_status set_dq_smem(KernelT kern, size_t bytes) {
+  GP_CUDA_OK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  return GP_OK;
+}
+
+template <int K, int D>
+static gp_status launch_logdet_grad_pk(const OpCtx& c) {
+  int64_t cnt = c.g->n - c.g->n0;
+  if (cnt <= 0) return GP_OK;
+  unsigned grid = (unsigned)((cnt + kGradThreads - 1) / kGradThreads);
+  KParams<float> kp = make_kparams<float>(*c.kern);
+  const Rec<float>* rec = (const Rec<float>*)c.rec();
+  size_t smem = dq_smem_bytes(K, kGradThreads);
+#define GP_LD(KIND)                                                                                              \
+  GP_OK_OR_RETURN(set_dq_smem(logdet_grad_pk_kernel<K, D, KIND>, smem));                                        \
+  logdet_grad_pk_kernel<K, D, KIND><<<grid, kGradThreads, smem, c.st>>>(rec, c.g->nbr, c.g->n0, c.g->n, c.g->n0, kp, c.ctrl());
+  switch (c.kern->kind) {
+    case GP_KERNEL_SE: GP_LD(GP_KERNEL_SE) break;
+    case GP_KERNEL_MATERN32: GP_LD(GP_KERNEL_MATERN32) break;
+    default: GP_LD(GP_KERNEL_EXP) break;
+  }
+#undef GP_LD
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+template <int K, int D>
+static gp_status launch_vjp_flow(const OpCtx& c, const float* xi, float* gbar, float* xibar) {
+  const int L = c.g->n_batches;
+  if (L <= 0) return GP_OK;
+  // device table: batch_off [L + 1], then the chunk prefix of the batches in REVERSE order [L + 1]
+  std::vector<int64_t> tab(2 * ((size_t)L + 1));
+  const int64_t* off = c.g->batch_off;
+  for (int b = 0; b <= L; ++b) tab[b] = off[b];
+  int64_t* cs = tab.data() + (L + 1);
+  cs[0] = 0;
+  for (int rb = 0; rb < L; ++rb) {
+    int b = L - 1 - rb;
+    cs[rb + 1] = cs[rb] + (off[b + 1] - off[b] + kGradThreads - 1) / kGradThreads;
+  }
+  const int64_t chunks = cs[L];
+  if (chunks <= 0 || chunks > 0x7fffffffLL) return GP_ERR_UNSUPPORTED;
+  // pageable source: the runtime stages it before returning, so the vector may die afterwards
+  GP_CUDA_OK(cudaMemcpyAsync(c.boff_dev(), tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, c.st));
+  KParams<float> kp = make_kparams<float>(*c.kern);
+  const Rec<float>* rec = (const Rec<float>*)c.rec();
+  const int64_t* boff_d = c.boff_dev();
+  const int64_t* cs_d = boff_d + (L + 1);
+  size_t smem = dq_smem_bytes(K, kGradThreads);
+#define GP_VF(KIND)                                                                                              \
+  GP_OK_OR_RETURN(set_dq_smem(vjp_flow_kernel<K, D, KIND>, smem));                                              \
+  vjp_flow_kernel<K, D, KIND><<<(unsigned)chunks, kGradThreads, smem, c.st>>>(rec, c.g->nbr, xi, gbar, xibar, boff_d, cs_d, L, \
+                                                                          c.g->n0, c.g->n, kp, c.ctrl());
+  switch (c.kern->kind) {
+    case GP_KERNEL_SE: GP_VF(GP_KERNEL_SE) break;
+    case GP_KERNEL_MATERN32: GP_VF(GP_KERNEL_MATERN32) break;
+    default: GP_VF(GP_KERNEL_EXP) break;
+  }
+#undef GP_VF
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+// (K, D) pairs with packed fp32 gradient kernels (K even)
+#define GP_GRAD_PK_TABLE(X) X(8, 3) X(16, 3) X(8, 2) X(16, 2)
+
 template <typename T>
 static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T* xibar, double* thetabar) {
   bool spec = grad_use_spec(c);
@@ -293,9 +506,20 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
     GP_OK_OR_RETURN(head_factor(hc, nullptr, 2 * (int)n0, true));
   }
   if (spec) GP_OK_OR_RETURN(grad_pack<T>(c, v));
-  const int64_t* off = c.g->batch_off;
-  for (int b = c.g->n_batches - 1; b >= 0; --b)
-    GP_OK_OR_RETURN((launch_grad_range<T, GRAD_VJP>(c, spec, v, xi, gbar, xibar, off[b], off[b + 1])));
+  bool flowed = false;
+  if constexpr (std::is_same<T, float>::value) {
+    if (spec && !(c.g->flags & GP_FLAG_PER_BATCH_LAUNCH)) {
+#define X(K, D) \
+      if (!flowed && c.g->k == K && c.g->d == D) { GP_OK_OR_RETURN((launch_vjp_flow<K, D>(c, xi, gbar, xibar))); flowed = true; }
+      GP_GRAD_PK_TABLE(X)
+#undef X
+    }
+  }
+  if (!flowed) {
+    const int64_t* off = c.g->batch_off;
+    for (int b = c.g->n_batches - 1; b >= 0; --b)
+      GP_OK_OR_RETURN((launch_grad_range<T, GRAD_VJP>(c, spec, v, xi, gbar, xibar, off[b], off[b + 1])));
+  }
   GP_OK_OR_RETURN(side_join(side, c.st));
   if (n0 > 0) GP_OK_OR_RETURN(head_vjp(c, xi, gbar, xibar, &c.ctrl()->acc[3]));
   finalize_grad_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), 3, 4, 1.0 / c.kern->ell, thetabar);
@@ -312,6 +536,14 @@ gp_status run_vjp(const OpCtx& c, const void* xi, const void* v, const void* vba
 template <typename T>
 static gp_status logdet_grad_t(const OpCtx& c) {
   bool spec = grad_use_spec(c);
+  if constexpr (std::is_same<T, float>::value) {
+    if (spec) {
+#define X(K, D) \
+      if (c.g->k == K && c.g->d == D) return launch_logdet_grad_pk<K, D>(c);
+      GP_GRAD_PK_TABLE(X)
+#undef X
+    }
+  }
   return launch_grad_range<T, GRAD_LOGDET>(c, spec, nullptr, nullptr, nullptr, nullptr, c.g->n0, c.g->n);
 }
 gp_status run_logdet_grad(const OpCtx& c) {
