@@ -12,7 +12,8 @@ namespace gp {
 
 constexpr int kMaxK = 64;
 constexpr int kMaxD = 4;
-constexpr int kCtrlBytes = 512;
+constexpr int kCtrlBytes = 2048;
+constexpr int kAccSlots = 64;
 constexpr int kMaxBatches = 1 << 20;
 
 // First kCtrlBytes of every workspace; zeroed by the library at the start of each op.
@@ -24,6 +25,7 @@ struct Control {
   double acc[8];               // [0] logdet  [1] dlogdet/dsigma  [2] dlogdet/dell  [3] theta_bar sigma  [4] theta_bar ell
   double build_ms[4];          // graph builder stage times
   unsigned long long pad[4];
+  double slots[2][kAccSlots];  // dataflow VJP: per-warp partial sums of sigma_bar / ell_bar, spread to avoid one hot address
 };
 static_assert(sizeof(Control) <= kCtrlBytes, "control block");
 
@@ -167,12 +169,12 @@ inline size_t dtype_bytes(int dtype) { return dtype == GP_F64 ? 8 : 4; }
 
 // Workspace layout (byte offsets from ws).  The head is always factored in fp64.
 //   ctrl     Control
-//   boff     device copy of batch_off (int64 [n_batches + 1]) + chunk prefix (int64 [n_batches + 1])
+//   boff     dataflow VJP: per batch in reverse order {first chunk, first point, end point, end chunk} (int64 x 4)
 //   head     (n0 + carried) x n0 doubles: factor of K_head/sigma^2 + carried rows (+ n0 doubles for the VJP)
 //   rec      packed records Rec<T>[n]                          (register-resident kernels only)
 //   g        VJP: running cotangent, T[n]
 struct WsLayout {
-  size_t ctrl_off, boff_off, head_off, rec_off, g_off, total;
+  size_t ctrl_off, boff_off, head_off, rec_off, g_off, wbuf_off, total;
   size_t head_rows;
 };
 inline WsLayout ws_layout(const gp_graph* g, int op) {
@@ -181,7 +183,7 @@ inline WsLayout ws_layout(const gp_graph* g, int op) {
   size_t n0 = (size_t)g->n0, n = (size_t)g->n;
   size_t off = 0;
   w.ctrl_off = off; off += kCtrlBytes;
-  w.boff_off = off; off += align_up(2 * ((size_t)g->n_batches + 1) * sizeof(int64_t), 256);
+  w.boff_off = off; off += align_up(4 * ((size_t)g->n_batches + 1) * sizeof(int64_t), 256);
   // carried rows: inverse 1 (v_head); gradients 2 n0 (identity -> L^-T, and ell dM/dell -> its L^-1 image)
   size_t carried = (op == GP_OP_INVERSE) ? 1 : (op == GP_OP_VJP ? 2 * n0 : 0);
   w.head_rows = n0 + carried;
@@ -191,6 +193,9 @@ inline WsLayout ws_layout(const gp_graph* g, int op) {
   w.rec_off = off; off += align_up(n * 4 * B, 256);
   w.g_off = off;
   if (op == GP_OP_VJP) off += align_up(n * B, 256);
+  // two-phase VJP (fp32): per conditioned point the k weights and {s, A_i, B_i, ok}
+  w.wbuf_off = off;
+  if (op == GP_OP_VJP && g->dtype == GP_F32) off += align_up((n - n0) * ((size_t)g->k + 4) * sizeof(float), 256);
   w.total = off;
   return w;
 }
@@ -206,6 +211,7 @@ struct OpCtx {
   double* head() const { return (double*)(ws + lay.head_off); }
   void* rec() const { return ws + lay.rec_off; }
   void* gbar() const { return ws + lay.g_off; }
+  float* wbuf() const { return (float*)(ws + lay.wbuf_off); }
 };
 
 // Fork/join helper: the dense head is independent of the bulk conditioning in gp_inverse / gp_logdet / gp_vjp,

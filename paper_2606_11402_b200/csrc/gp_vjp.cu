@@ -183,46 +183,76 @@ logdet_grad_pk_kernel(const Rec<float>* __restrict__ rec, const int32_t* __restr
   block_atomic_add(acc_ell, &ctrl->acc[2], red);
 }
 
-// VJP of the forward pass in ONE launch, batches in reverse order.  CTAs take batch-aligned chunks through a
-// ticket (last batch first).  A chunk of batch b may read its cotangents once every point of every later batch
-// has scattered: ctrl->done counts finished points, so the test is done >= n - batch_off[b + 1].  Lower tickets
-// have always started and never wait on higher ones, so polling cannot deadlock.
+// VJP of the forward pass in two launches.
+//  (1) vjp_geom_kernel: everything that does not depend on the incoming cotangent, for all points at once (no
+//      ordering constraint, register-heavy): writes the k weights and {s, A_i, B_i, ok} of every point.
+//  (2) vjp_scatter_kernel: the reverse sweep proper, a light kernel at full occupancy.  CTAs take batch-aligned
+//      chunks through a ticket, last batch first.  A chunk of batch b may read its cotangents once every point
+//      of every later batch has scattered: ctrl->done counts finished points (done >= n - batch_off[b + 1]).
+//      Lower tickets have always started and never wait on higher ones, so polling cannot deadlock.
 template <int K, int D, int KIND>
 __global__ void __launch_bounds__(kGradThreads, GP_GRAD_MIN_CTAS)
-vjp_flow_kernel(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ nbr, const float* __restrict__ xi,
-                float* gbar, float* __restrict__ xibar, const int64_t* __restrict__ boff,
-                const int64_t* __restrict__ cstart, int L, int64_t n0, int64_t n, KParams<float> kp, Control* ctrl) {
+vjp_geom_kernel(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ nbr, const float* __restrict__ xi,
+                float* __restrict__ wbuf, float4* __restrict__ sab, int64_t n0, int64_t n, KParams<float> kp,
+                Control* ctrl) {
   extern __shared__ float4 dq_raw[];
+  const int64_t i = n0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  DqStore<K> dq = dq_store_of<K>(dq_raw);
+  Rec<float> self = load_rec<false>(rec + i);
+  f2 W[K / 2], AL[K / 2];
+  float s;
+  bool ok = grad_geometry_pk<K, D, KIND>(rec, nbr + (i - n0) * K, self, kp, dq, W, AL, s);
+  const float xi_i = xi[i];
+  const float Ai = grad_sweep_pk<K>(W, AL, kp.sigma * xi_i / s, dq);
+  if (!ok) atomicAdd(&ctrl->n_bad, 1ULL);
+  float4* wrow = reinterpret_cast<float4*>(wbuf + (i - n0) * K);
+#pragma unroll
+  for (int q = 0; q < K / 4; ++q) wrow[q] = make_float4(W[2 * q].x, W[2 * q].y, W[2 * q + 1].x, W[2 * q + 1].y);
+  sab[i - n0] = make_float4(s, Ai, s * xi_i, ok ? 1.0f : 0.0f);
+}
+
+constexpr int kScatterThreads = 256;
+
+template <int K>
+__global__ void __launch_bounds__(kScatterThreads, 4)
+vjp_scatter_kernel(const int32_t* __restrict__ nbr, const float* __restrict__ wbuf, const float4* __restrict__ sab,
+                   float* gbar, float* __restrict__ xibar, const longlong4* __restrict__ tab, int L, int64_t n0,
+                   int64_t n, float sigma, Control* ctrl) {
   __shared__ double red[32];
   __shared__ long long s_info[3];
-  if (threadIdx.x == 0) {
-    long long t = (long long)atomicAdd(&ctrl->ticket, 1ULL);
-    int lo = 0, hi = L - 1;                      // largest rb with cstart[rb] <= t
-    while (lo < hi) {
-      int mid = (lo + hi + 1) >> 1;
-      if (cstart[mid] <= t) lo = mid; else hi = mid - 1;
+  __shared__ long long s_ticket;
+  if (threadIdx.x == 0) s_ticket = (long long)atomicAdd(&ctrl->ticket, 1ULL);
+  __syncthreads();
+  {
+    const long long t = s_ticket;
+    for (int q = threadIdx.x; q < L; q += blockDim.x) {
+      const longlong2 e01 = __ldg(reinterpret_cast<const longlong2*>(tab + q));
+      const longlong2 e23 = __ldg(reinterpret_cast<const longlong2*>(tab + q) + 1);
+      if (e01.x <= t && t < e23.y) {   // {first chunk, first point, end point, end chunk} of reverse batch q
+        s_info[0] = e01.y + (t - e01.x) * (long long)blockDim.x;
+        s_info[1] = e23.x;
+        s_info[2] = n - e23.x;
+      }
     }
-    int b = L - 1 - lo;
-    s_info[0] = boff[b] + (t - cstart[lo]) * (long long)blockDim.x;
-    s_info[1] = boff[b + 1];
-    s_info[2] = n - boff[b + 1];
   }
   __syncthreads();
   const int64_t i = s_info[0] + threadIdx.x;
   const int64_t end = s_info[1];
   const bool active = i < end;
-  const int32_t* row = nbr + (i - n0) * K;
-  f2 W[K / 2];
-  float s = 0.0f, Ai = 0.0f, Bi = 0.0f;
-  bool ok = true;
+  // everything that does not depend on the cotangent is fetched before waiting
+  int32_t idx[K];
+  float w[K];
+  float4 q4 = make_float4(0.f, 0.f, 0.f, 0.f);
   if (active) {
-    DqStore<K> dq = dq_store_of<K>(dq_raw);
-    Rec<float> self = load_rec<false>(rec + i);
-    f2 AL[K / 2];
-    ok = grad_geometry_pk<K, D, KIND>(rec, row, self, kp, dq, W, AL, s);
-    const float xi_i = xi[i];
-    Ai = grad_sweep_pk<K>(W, AL, kp.sigma * xi_i / s, dq);
-    Bi = s * xi_i;
+    load_row<K>(nbr + (i - n0) * K, idx);
+    const float4* wrow = reinterpret_cast<const float4*>(wbuf + (i - n0) * K);
+#pragma unroll
+    for (int q = 0; q < K / 4; ++q) {
+      float4 t = __ldcs(wrow + q);
+      w[4 * q] = t.x; w[4 * q + 1] = t.y; w[4 * q + 2] = t.z; w[4 * q + 3] = t.w;
+    }
+    q4 = __ldcs(sab + (i - n0));
   }
   if (threadIdx.x == 0) {
     const unsigned long long need = (unsigned long long)s_info[2];
@@ -230,37 +260,33 @@ vjp_flow_kernel(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ 
     unsigned spins = 0;
     while (true) {
       unsigned long long d;
-      asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(d) : "l"(&ctrl->done) : "memory");
+      asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(d) : "l"(&ctrl->done) : "memory");
       if (d >= need) break;
-      if (++spins > 4) __nanosleep(64);
+      if (++spins > 16) __nanosleep(32);
       if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) { atomicAdd(&ctrl->timeout, 1ULL); break; }
     }
   }
   __syncthreads();
   double acc_sigma = 0.0, acc_ell = 0.0;
   if (active) {
-    const float g = __ldcg(gbar + i);
-    float out = kp.sigma * g * s;
-    if (!ok) { atomicAdd(&ctrl->n_bad, 1ULL); out = qnan<float>(); }
-    xibar[i] = out;
+    const float g = __ldcg(gbar + i);           // L2: the cotangent was accumulated there by atomics
+    const bool ok = q4.w != 0.0f;
+    xibar[i] = ok ? sigma * g * q4.x : qnan<float>();
     if (ok) {
-      int32_t idx[K];
-      load_row<K>(row, idx);
 #pragma unroll
-      for (int rp = 0; rp < K / 2; ++rp) {
-        atomicAdd(gbar + idx[2 * rp], g * W[rp].x);
-        atomicAdd(gbar + idx[2 * rp + 1], g * W[rp].y);
-      }
-      acc_sigma = (double)(g * Bi);
-      acc_ell = (double)(g * Ai);
+      for (int j = 0; j < K; ++j) atomicAdd(gbar + idx[j], g * w[j]);
+      acc_sigma = (double)(g * q4.z);
+      acc_ell = (double)(g * q4.y);
     }
   }
-  __threadfence();
-  block_atomic_add(acc_sigma, &ctrl->acc[3], red);
-  block_atomic_add(acc_ell, &ctrl->acc[4], red);
+  // block sums (their barriers also order every thread's scatter before thread 0's fence below)
+  const int slot = (int)(blockIdx.x % kAccSlots);
+  block_atomic_add(acc_sigma, &ctrl->slots[0][slot], red);
+  block_atomic_add(acc_ell, &ctrl->slots[1][slot], red);
   if (threadIdx.x == 0) {
     long long cnt = end - s_info[0];
     if (cnt > (long long)blockDim.x) cnt = blockDim.x;
+    __threadfence();
     atomicAdd(&ctrl->done, (unsigned long long)cnt);
   }
 }
@@ -417,8 +443,10 @@ static gp_status grad_pack(const OpCtx& c, const T* vals) {
 // theta_bar[0] = sigma_bar, theta_bar[1] = ell_bar; the kernels accumulate ell * d/dell
 __global__ void finalize_grad_kernel(const Control* ctrl, int slot_sigma, int slot_ell, double inv_ell, double* out2) {
   if (threadIdx.x == 0 && blockIdx.x == 0) {
-    out2[0] = ctrl->acc[slot_sigma];
-    out2[1] = ctrl->acc[slot_ell] * inv_ell;
+    double a = ctrl->acc[slot_sigma], b = ctrl->acc[slot_ell];
+    for (int q = 0; q < kAccSlots; ++q) { a += ctrl->slots[0][q]; b += ctrl->slots[1][q]; }
+    out2[0] = a;
+    out2[1] = b * inv_ell;
   }
 }
 
@@ -452,36 +480,43 @@ static gp_status launch_logdet_grad_pk(const OpCtx& c) {
 template <int K, int D>
 static gp_status launch_vjp_flow(const OpCtx& c, const float* xi, float* gbar, float* xibar) {
   const int L = c.g->n_batches;
-  if (L <= 0) return GP_OK;
-  // device table: batch_off [L + 1], then the chunk prefix of the batches in REVERSE order [L + 1]
-  std::vector<int64_t> tab(2 * ((size_t)L + 1));
+  const int64_t cnt = c.g->n - c.g->n0;
+  if (L <= 0 || cnt <= 0) return GP_OK;
+  // device table, one entry per batch in REVERSE order: {first chunk, first point, end point, end chunk}
+  std::vector<int64_t> tab(4 * (size_t)L);
   const int64_t* off = c.g->batch_off;
-  for (int b = 0; b <= L; ++b) tab[b] = off[b];
-  int64_t* cs = tab.data() + (L + 1);
-  cs[0] = 0;
+  int64_t chunks = 0;
   for (int rb = 0; rb < L; ++rb) {
     int b = L - 1 - rb;
-    cs[rb + 1] = cs[rb] + (off[b + 1] - off[b] + kGradThreads - 1) / kGradThreads;
+    int64_t nc = (off[b + 1] - off[b] + kScatterThreads - 1) / kScatterThreads;
+    tab[4 * rb + 0] = chunks;
+    tab[4 * rb + 1] = off[b];
+    tab[4 * rb + 2] = off[b + 1];
+    tab[4 * rb + 3] = chunks + nc;
+    chunks += nc;
   }
-  const int64_t chunks = cs[L];
   if (chunks <= 0 || chunks > 0x7fffffffLL) return GP_ERR_UNSUPPORTED;
   // pageable source: the runtime stages it before returning, so the vector may die afterwards
   GP_CUDA_OK(cudaMemcpyAsync(c.boff_dev(), tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, c.st));
   KParams<float> kp = make_kparams<float>(*c.kern);
   const Rec<float>* rec = (const Rec<float>*)c.rec();
-  const int64_t* boff_d = c.boff_dev();
-  const int64_t* cs_d = boff_d + (L + 1);
+  const longlong4* tab_d = (const longlong4*)c.boff_dev();
+  float* wbuf = c.wbuf();
+  float4* sab = reinterpret_cast<float4*>(wbuf + (size_t)cnt * K);
   size_t smem = dq_smem_bytes(K, kGradThreads);
+  unsigned ggrid = (unsigned)((cnt + kGradThreads - 1) / kGradThreads);
 #define GP_VF(KIND)                                                                                              \
-  GP_OK_OR_RETURN(set_dq_smem(vjp_flow_kernel<K, D, KIND>, smem));                                              \
-  vjp_flow_kernel<K, D, KIND><<<(unsigned)chunks, kGradThreads, smem, c.st>>>(rec, c.g->nbr, xi, gbar, xibar, boff_d, cs_d, L, \
-                                                                          c.g->n0, c.g->n, kp, c.ctrl());
+  GP_OK_OR_RETURN(set_dq_smem(vjp_geom_kernel<K, D, KIND>, smem));                                              \
+  vjp_geom_kernel<K, D, KIND><<<ggrid, kGradThreads, smem, c.st>>>(rec, c.g->nbr, xi, wbuf, sab, c.g->n0, c.g->n, kp, c.ctrl());
   switch (c.kern->kind) {
     case GP_KERNEL_SE: GP_VF(GP_KERNEL_SE) break;
     case GP_KERNEL_MATERN32: GP_VF(GP_KERNEL_MATERN32) break;
     default: GP_VF(GP_KERNEL_EXP) break;
   }
 #undef GP_VF
+  GP_LAUNCH_CHECK();
+  vjp_scatter_kernel<K><<<(unsigned)chunks, kScatterThreads, 0, c.st>>>(c.g->nbr, wbuf, sab, gbar, xibar, tab_d, L, c.g->n0,
+                                                                      c.g->n, kp.sigma, c.ctrl());
   GP_LAUNCH_CHECK();
   return GP_OK;
 }
