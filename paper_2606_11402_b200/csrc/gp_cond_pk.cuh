@@ -120,15 +120,12 @@ __device__ __forceinline__ bool factor_joint_pk(f2 (&P)[pk_pairs(K)], float diag
   return (minpiv > 0.0f) && (s2 < 3.0e38f);
 }
 
-// forward / inverse / logdet body: gather, build, factor.
-template <int K, int D, int KIND, bool COHERENT>
-__device__ __forceinline__ Cond<float> condition_pk(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ row,
-                                                    const Rec<float>& self, const KParams<float>& kp) {
+// forward / inverse / logdet body on gathered records: build, factor.
+template <int K, int D, int KIND>
+__device__ __forceinline__ Cond<float> condition_pk_rec(const Rec<float> (&R)[K], const Rec<float>& self,
+                                                        const KParams<float>& kp) {
   f2 P[pk_pairs(K)];
   {
-    int32_t idx[K];
-    Rec<float> R[K];
-    gather_reg<float, K, COHERENT>(rec, row, idx, R);
     PkCoords<K> X;
     centre_pk<K, D>(R, self, kp.sq, X);
     float vals[K];
@@ -141,6 +138,15 @@ __device__ __forceinline__ Cond<float> condition_pk(const Rec<float>* __restrict
   out.m = -P[pk(K / 2, K)].y;
   out.s = Math<float>::sqrt(P[pk(K / 2, K)].x);
   return out;
+}
+
+template <int K, int D, int KIND, bool COHERENT>
+__device__ __forceinline__ Cond<float> condition_pk(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ row,
+                                                    const Rec<float>& self, const KParams<float>& kp) {
+  int32_t idx[K];
+  Rec<float> R[K];
+  gather_reg<float, K, COHERENT>(rec, row, idx, R);
+  return condition_pk_rec<K, D, KIND>(R, self, kp);
 }
 
 // v-independent half for the dataflow forward: weights w = L_cc^-T l (= K_cc^-1 K_ci, Eq. 2) and s.
