@@ -1,0 +1,97 @@
+// Lane-group conditioning: one point split over L consecutive lanes of a warp (PAPER.md:53 says the register
+// budget (k+1)[d+1+(k+2)/2] limits one thread to k <~ 64 on the paper's GPU; on sm_100a one thread per point
+// stops paying at k = 16 in fp32 and k = 8 in fp64: 255 registers).  Used for k = 32 fp32 and k = 16 fp64.
+//
+// Rows of the joint matrix plus the carried values row - K + 2 rows, row K
+// the point itself, row K + 1 the values - are dealt cyclically to the lanes: row r lives in lane r % L, slot
+// r / L, so every register index below is a compile-time constant and nothing spills.  A right-looking step j
+// needs L[c][j] for all c > j in every lane: one width-L shuffle per (j, c) from the lane that owns row c.
+// Entries above the diagonal inside a slot are computed as harmless finite junk and never read.
+#pragma once
+#include "gp_cond.cuh"
+
+namespace gp {
+
+template <typename T> __device__ __forceinline__ T shfl_grp(T v, int src, int width) {
+  return __shfl_sync(0xffffffffu, v, src, width);
+}
+
+template <typename T, int K, int L> struct LgShape {
+  static constexpr int ROWS = K + 2;
+  static constexpr int S = (ROWS + L - 1) / L;
+  // columns a slot needs: rows of slot s reach s L + L - 1, capped at K
+  __host__ __device__ static constexpr int cols(int s) { return (s * L + L - 1 < K ? s * L + L - 1 : K) + 1; }
+};
+
+// Result in every lane of the group: m, s (unit sigma), ok, and the point's own value.
+template <typename T> struct LgCond { T m, s, self_v; bool ok; };
+
+template <typename T, int K, int D, int KIND, int L, bool COHERENT>
+__device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ row,
+                                                  int64_t i, int l, const KParams<T>& kp) {
+  using Sh = LgShape<T, K, L>;
+  constexpr int S = Sh::S;
+  T X0[S], X1[S], X2[S], V[S];
+#pragma unroll
+  for (int s = 0; s < S; ++s) {
+    const int r = s * L + l;
+    Rec<T> R;
+    R.x0 = R.x1 = R.x2 = R.v = T(0);
+    if (r < K) R = load_rec<COHERENT>(rec + row[r]);
+    else if (r == K) R = load_rec<COHERENT>(rec + i);
+    X0[s] = R.x0; X1[s] = R.x1; X2[s] = R.x2; V[s] = R.v;
+  }
+  // a[s][c], c < cols(s); flattened with a fixed stride so that the indices stay compile-time
+  T a[S][K + 1];
+#pragma unroll
+  for (int c = 0; c < K; ++c) {
+    const int cs = c / L, co = c % L;
+    const T c0 = shfl_grp(X0[cs], co, L);
+    const T c1 = D >= 2 ? shfl_grp(X1[cs], co, L) : T(0);
+    const T c2 = D >= 3 ? shfl_grp(X2[cs], co, L) : T(0);
+    const T vc = shfl_grp(V[cs], co, L);
+#pragma unroll
+    for (int s = cs; s < S; ++s) {
+      const int r = s * L + l;
+      T dx = X0[s] - c0;
+      T d2 = dx * dx;
+      if (D >= 2) { T dy = X1[s] - c1; d2 = Math<T>::fma(dy, dy, d2); }
+      if (D >= 3) { T dz = X2[s] - c2; d2 = Math<T>::fma(dz, dz, d2); }
+      const T rho = Math<T>::template rho_from_q<KIND>(d2 * kp.qscale);
+      T val = T(0);
+      if (r > c) val = (r == K + 1) ? vc : rho;
+      else if (r == c) val = kp.diag;
+      a[s][c] = val;
+    }
+  }
+#pragma unroll
+  for (int s = K / L; s < S; ++s) a[s][K] = (s * L + l == K) ? kp.diag : T(0);
+
+  T minpiv = kp.diag;
+#pragma unroll
+  for (int j = 0; j < K; ++j) {
+    const int js = j / L, jo = j % L;
+    const T piv = shfl_grp(a[js][j], jo, L);
+    minpiv = Math<T>::fmin(minpiv, piv);
+    const T inv = Math<T>::rsqrt(piv);
+#pragma unroll
+    for (int s = js; s < S; ++s) a[s][j] *= inv;
+#pragma unroll
+    for (int c = j + 1; c <= K; ++c) {
+      const T lc = shfl_grp(a[c / L][j], c % L, L);
+#pragma unroll
+      for (int s = c / L; s < S; ++s) a[s][c] = Math<T>::fma(-a[s][j], lc, a[s][c]);
+    }
+  }
+  LgCond<T> out;
+  const T s2 = shfl_grp(a[K / L][K], K % L, L);
+  const T negm = shfl_grp(a[(K + 1) / L][K], (K + 1) % L, L);
+  out.self_v = shfl_grp(V[K / L], K % L, L);
+  minpiv = Math<T>::fmin(minpiv, s2);
+  out.ok = (minpiv > T(0)) && (s2 == s2) && (s2 < T(3.0e38));
+  out.m = -negm;
+  out.s = Math<T>::sqrt(s2);
+  return out;
+}
+
+}  // namespace gp

@@ -4,6 +4,7 @@
 //   logdet   PAPER.md:9:  sum_i log s_i^2, fp64 accumulation
 #include <type_traits>
 
+#include "gp_cond_lg.cuh"
 #include "gp_cond_pk.cuh"
 
 namespace gp {
@@ -83,6 +84,38 @@ cond_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* 
       rec[i].v = v;
     } else if (OP == OPK_INVERSE) {
       T xi = (self.v - c.m) / ss;
+      if (!c.ok) xi = quiet_nan<T>();
+      out[i] = xi;
+    } else {
+      ld = c.ok ? 2.0 * (double)Math<T>::log(ss) : 0.0;
+    }
+  }
+  if (OP == OPK_LOGDET) block_atomic_add(ld, &ctrl->acc[0], red);
+}
+
+// ---- lane-group kernel: one point per L lanes (k = 32 fp32, k = 16 fp64) -----------------------------------
+template <typename T, int K, int D, int KIND, int L, int OP>
+__global__ void __launch_bounds__(kCondThreads)
+cond_lg_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* __restrict__ in, T* __restrict__ out,
+               int64_t start, int64_t end, int64_t n0, KParams<T> kp, Control* ctrl) {
+  __shared__ double red[32];
+  constexpr int PPB = kCondThreads / L;
+  const int l = threadIdx.x % L;
+  int64_t i = start + (int64_t)blockIdx.x * PPB + threadIdx.x / L;
+  const bool live = i < end;
+  if (!live) i = end - 1;                     // every lane takes part in the shuffles; the result is dropped
+  LgCond<T> c = condition_lg<T, K, D, KIND, L, false>(rec, nbr + (i - n0) * K, i, l, kp);
+  double ld = 0.0;
+  if (live && l == 0) {
+    const T ss = kp.sigma * c.s;
+    if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
+    if (OP == OPK_FORWARD) {
+      T v = Math<T>::fma(ss, in[i], c.m);
+      if (!c.ok) v = quiet_nan<T>();
+      out[i] = v;
+      rec[i].v = v;
+    } else if (OP == OPK_INVERSE) {
+      T xi = (c.self_v - c.m) / ss;
       if (!c.ok) xi = quiet_nan<T>();
       out[i] = xi;
     } else {
@@ -208,8 +241,15 @@ int generic_active_threads(int k, size_t elem_bytes, bool with_vjp) {
 #define GP_SPEC_TABLE(X) \
   X(float, 8, 3) X(float, 16, 3) X(float, 8, 2) X(float, 16, 2) X(double, 8, 3) X(double, 8, 2)
 
+// (dtype, K, D, L): lane-group kernels
+#define GP_LG_TABLE(X) X(float, 32, 2, 8) X(float, 32, 3, 8) X(double, 16, 3, 4) X(double, 16, 2, 4)
+
 bool has_specialised(int dtype, int k, int d, int kind) {
   if (kind < 0 || kind > 2) return false;
+#define X(T, K, D, L) \
+  if ((dtype == GP_F64) == (sizeof(T) == 8) && k == K && d == D) return true;
+  GP_LG_TABLE(X)
+#undef X
 #define X(T, K, D) \
   if ((dtype == GP_F64) == (sizeof(T) == 8) && k == K && d == D) return true;
   GP_SPEC_TABLE(X)
@@ -233,6 +273,29 @@ static gp_status launch_spec_kind(const OpCtx& c, const T* in, T* out, int64_t s
       break;
     default:
       cond_kernel<T, K, D, GP_KERNEL_EXP, OP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, in, out, start, end, c.g->n0, kp, c.ctrl());
+      break;
+  }
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+template <typename T, int K, int D, int L, int OP>
+static gp_status launch_lg(const OpCtx& c, const T* in, T* out, int64_t start, int64_t end) {
+  int64_t cnt = end - start;
+  if (cnt <= 0) return GP_OK;
+  constexpr int PPB = kCondThreads / L;
+  unsigned grid = (unsigned)((cnt + PPB - 1) / PPB);
+  KParams<T> kp = make_kparams<T>(*c.kern);
+  Rec<T>* rec = (Rec<T>*)c.rec();
+  switch (c.kern->kind) {
+    case GP_KERNEL_SE:
+      cond_lg_kernel<T, K, D, GP_KERNEL_SE, L, OP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, in, out, start, end, c.g->n0, kp, c.ctrl());
+      break;
+    case GP_KERNEL_MATERN32:
+      cond_lg_kernel<T, K, D, GP_KERNEL_MATERN32, L, OP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, in, out, start, end, c.g->n0, kp, c.ctrl());
+      break;
+    default:
+      cond_lg_kernel<T, K, D, GP_KERNEL_EXP, L, OP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, in, out, start, end, c.g->n0, kp, c.ctrl());
       break;
   }
   GP_LAUNCH_CHECK();
@@ -274,6 +337,12 @@ static gp_status launch_range(const OpCtx& c, bool spec, const T* vals, const T*
       if (c.g->k == K && c.g->d == D) return launch_spec_kind<T, K, D, OP>(c, in, out, start, end); \
     }
     GP_SPEC_TABLE(X)
+#undef X
+#define X(TT, K, D, L) \
+    if constexpr (std::is_same<TT, T>::value) {                    \
+      if (c.g->k == K && c.g->d == D) return launch_lg<T, K, D, L, OP>(c, in, out, start, end); \
+    }
+    GP_LG_TABLE(X)
 #undef X
   }
   return launch_generic<T, OP>(c, vals, in, out, start, end);
@@ -323,7 +392,13 @@ static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
 template <typename T>
 static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
   bool spec = use_spec(c);
-  bool flow = spec && !(c.g->flags & GP_FLAG_PER_BATCH_LAUNCH);
+  bool flow = false;                          // single-launch dataflow: one-thread-per-point shapes only
+  if (spec && !(c.g->flags & GP_FLAG_PER_BATCH_LAUNCH)) {
+#define X(TT, K, D) \
+    if (std::is_same<TT, T>::value && c.g->k == K && c.g->d == D) flow = true;
+    GP_SPEC_TABLE(X)
+#undef X
+  }
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
   // the head is on the critical path (every batch depends on it); packing the records is not: side stream
   SideStream* side = nullptr;
