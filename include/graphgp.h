@@ -45,7 +45,10 @@ typedef enum { GP_OP_FORWARD = 0, GP_OP_INVERSE = 1, GP_OP_LOGDET = 2, GP_OP_VJP
 enum {
   GP_FLAG_PER_BATCH_LAUNCH = 1, /* forward/VJP: one launch per batch (Alg. 1 lines 2-8 literally) instead of
                                    the single dataflow launch; results agree to rounding */
-  GP_FLAG_GENERIC_KERNEL = 2    /* force the runtime-(k,d,kind) kernel even where a specialised one exists */
+  GP_FLAG_GENERIC_KERNEL = 2,   /* force the runtime-(k,d,kind) kernel even where a specialised one exists */
+  GP_FLAG_FLOW_CARRY = 4,       /* dataflow forward: use the wait-first body (meant for large batches) everywhere */
+  GP_FLAG_FLOW_WEIGHTS = 8      /* dataflow forward: use the wait-last body (meant for small batches) everywhere;
+                                   without either flag the library picks per stretch of batches by their size */
 };
 
 /* Stationary covariance kappa(r) = sigma^2 rho(r); rho:

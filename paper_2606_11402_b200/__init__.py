@@ -19,7 +19,7 @@ from .build import LIB, build_library
 GP_OK, GP_ERR_INVALID_ARG, GP_ERR_UNSUPPORTED, GP_ERR_NOT_PD, GP_ERR_CUDA, GP_ERR_WORKSPACE = range(6)
 GP_F32, GP_F64 = 0, 1
 GP_OP_FORWARD, GP_OP_INVERSE, GP_OP_LOGDET, GP_OP_VJP, GP_OP_BUILD = range(5)
-GP_FLAG_PER_BATCH_LAUNCH, GP_FLAG_GENERIC_KERNEL = 1, 2
+GP_FLAG_PER_BATCH_LAUNCH, GP_FLAG_GENERIC_KERNEL, GP_FLAG_FLOW_CARRY, GP_FLAG_FLOW_WEIGHTS = 1, 2, 4, 8
 GP_BUILD_SPATIAL_BATCHES = 1
 KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
 

@@ -134,61 +134,100 @@ cond_lg_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const 
 // ago and the first gather already returns them; only at the frontier (and in the small early batches, where
 // the per-batch latency chain of a launch-per-batch loop is what costs) does a thread poll.  The value word
 // is its own ready flag, so no fence or counter is involved.
-template <typename T, int K, int D, int KIND>
+//
+// Two bodies share the scheme.  FLOW_WEIGHTS (above) is for the stretches of SMALL batches, where the chain of
+// dependent batches is what costs: the wait comes last, after all the arithmetic.  FLOW_CARRY is for the
+// stretches of LARGE batches (larger than what the GPU holds in flight, so a neighbour is almost never
+// pending): it waits first - almost always zero iterations - and then runs exactly the inverse's body, values
+// row carried through the factorisation, no back-substitution.  The host cuts the graph
+// order into such stretches (at batch boundaries) and launches one kernel per stretch; tickets keep counting
+// across launches, `chunk0` is the number handed out before this launch.
+enum { FLOW_WEIGHTS = 0, FLOW_CARRY = 1 };
+
+template <typename T, int K>
+__device__ __forceinline__ bool wait_values(Rec<T>* rec, const int32_t (&idx)[K], T (&vv)[K], Control* ctrl) {
+  bool missing = false;
+#pragma unroll
+  for (int j = 0; j < K; ++j) missing |= Pending<T>::is(vv[j]);
+  if (!missing) return true;
+  const long long t0 = clock64();
+  unsigned spins = 0;
+  while (true) {
+    missing = false;
+#pragma unroll
+    for (int j = 0; j < K; ++j) {
+      if (Pending<T>::is(vv[j])) {
+        vv[j] = Pending<T>::load(&rec[idx[j]].v);
+        missing |= Pending<T>::is(vv[j]);
+      }
+    }
+    if (!missing) return true;
+    if (++spins > 8) __nanosleep(spins > 64 ? 256 : 32);
+    if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) {   // watchdog (about 4 s): a bug, never expected
+      atomicAdd(&ctrl->timeout, 1ULL);
+      return false;
+    }
+  }
+}
+
+template <typename T, int K, int D, int KIND, int MODE>
 __global__ void __launch_bounds__(kCondThreads, GP_FLOW_MIN_CTAS)
 forward_flow_kernel(Rec<T>* rec, const int32_t* __restrict__ nbr, const T* __restrict__ xi, T* __restrict__ out,
-                    int64_t n0, int64_t n, KParams<T> kp, Control* ctrl) {
+                    int64_t n0, int64_t first, int64_t end, unsigned long long chunk0, KParams<T> kp, Control* ctrl) {
   __shared__ unsigned long long s_chunk;
-  if (threadIdx.x == 0) s_chunk = atomicAdd(&ctrl->ticket, 1ULL);
+  if (threadIdx.x == 0) s_chunk = atomicAdd(&ctrl->ticket, 1ULL) - chunk0;
   __syncthreads();
-  const int64_t i = n0 + (int64_t)s_chunk * blockDim.x + threadIdx.x;
-  if (i >= n) return;
+  const int64_t i = first + (int64_t)s_chunk * blockDim.x + threadIdx.x;
+  if (i >= end) return;
   const int32_t* row = nbr + (i - n0) * K;
-  T w[K];
   Cond<T> c;
-  {
+  T m;
+  if (MODE == FLOW_CARRY) {
     Rec<T> self = load_rec_l1(rec + i);
     int32_t idx[K];
     Rec<T> R[K];
+    T vv[K];
     load_row<K>(row, idx);
 #pragma unroll
     for (int j = 0; j < K; ++j) R[j] = load_rec_l1(rec + idx[j]);
-    if constexpr (std::is_same<T, float>::value && K % 2 == 0) c = weights_pk<K, D, KIND>(R, self, kp, w);
-    else c = weights_reg<T, K, D, KIND>(R, self, kp, w);
-  }
-  // values: read again now (the lines are in L1 from the gather above; a stale "pending" is re-read from L2)
-  T vv[K];
-  {
+#pragma unroll
+    for (int j = 0; j < K; ++j) vv[j] = R[j].v;
+    bool got = wait_values<T, K>(rec, idx, vv, ctrl);
+#pragma unroll
+    for (int j = 0; j < K; ++j) R[j].v = vv[j];
+    if constexpr (std::is_same<T, float>::value && K % 2 == 0) {
+      c = condition_pk_rec<K, D, KIND>(R, self, kp);
+    } else {
+      T A[(K + 1) * (K + 2) / 2];
+      build_joint_reg<T, K, D, KIND>(R, self, kp, A);
+      c = factor_joint_reg<T, K, false>(A, vv, kp);
+    }
+    c.ok = c.ok && got;
+    m = c.m;
+  } else {
+    T w[K];
+    {
+      Rec<T> self = load_rec_l1(rec + i);
+      int32_t idx[K];
+      Rec<T> R[K];
+      load_row<K>(row, idx);
+#pragma unroll
+      for (int j = 0; j < K; ++j) R[j] = load_rec_l1(rec + idx[j]);
+      if constexpr (std::is_same<T, float>::value && K % 2 == 0) c = weights_pk<K, D, KIND>(R, self, kp, w);
+      else c = weights_reg<T, K, D, KIND>(R, self, kp, w);
+    }
+    // values: read again now (the lines are in L1 from the gather above; a stale "pending" is re-read from L2)
+    T vv[K];
     int32_t idx[K];
     load_row<K>(row, idx);
-    bool missing = false;
 #pragma unroll
-    for (int j = 0; j < K; ++j) { vv[j] = load_val_l1(&rec[idx[j]].v); missing |= Pending<T>::is(vv[j]); }
-    if (missing) {
-      const long long t0 = clock64();
-      unsigned spins = 0;
-      while (true) {
-        missing = false;
+    for (int j = 0; j < K; ++j) vv[j] = load_val_l1(&rec[idx[j]].v);
+    bool got = wait_values<T, K>(rec, idx, vv, ctrl);
+    c.ok = c.ok && got;
+    m = T(0);
 #pragma unroll
-        for (int j = 0; j < K; ++j) {
-          if (Pending<T>::is(vv[j])) {
-            vv[j] = Pending<T>::load(&rec[idx[j]].v);
-            missing |= Pending<T>::is(vv[j]);
-          }
-        }
-        if (!missing) break;
-        if (++spins > 8) __nanosleep(spins > 64 ? 256 : 32);
-        if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) {   // watchdog (about 4 s): a bug, never expected
-          atomicAdd(&ctrl->timeout, 1ULL);
-          c.ok = false;
-          break;
-        }
-      }
-    }
+    for (int j = 0; j < K; ++j) m = Math<T>::fma(w[j], vv[j], m);
   }
-  T m = T(0);
-#pragma unroll
-  for (int j = 0; j < K; ++j) m = Math<T>::fma(w[j], vv[j], m);
   T v = Math<T>::fma(kp.sigma * c.s, xi[i], m);
   if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
   if (!c.ok || v != v) v = quiet_nan<T>();
@@ -367,25 +406,59 @@ __global__ void finalize_logdet_kernel(const Control* ctrl, double* logdet, doub
   }
 }
 
-template <typename T, int K, int D>
-static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
-  int64_t cnt = c.g->n - c.g->n0;
+template <typename T, int K, int D, int MODE>
+static gp_status launch_flow_segment(const OpCtx& c, const T* xi, T* v, int64_t first, int64_t end, unsigned long long chunk0) {
+  int64_t cnt = end - first;
   if (cnt <= 0) return GP_OK;
   unsigned grid = (unsigned)((cnt + kCondThreads - 1) / kCondThreads);
   KParams<T> kp = make_kparams<T>(*c.kern);
   Rec<T>* rec = (Rec<T>*)c.rec();
   switch (c.kern->kind) {
     case GP_KERNEL_SE:
-      forward_flow_kernel<T, K, D, GP_KERNEL_SE><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, c.g->n, kp, c.ctrl());
+      forward_flow_kernel<T, K, D, GP_KERNEL_SE, MODE><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, first, end, chunk0, kp, c.ctrl());
       break;
     case GP_KERNEL_MATERN32:
-      forward_flow_kernel<T, K, D, GP_KERNEL_MATERN32><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, c.g->n, kp, c.ctrl());
+      forward_flow_kernel<T, K, D, GP_KERNEL_MATERN32, MODE><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, first, end, chunk0, kp, c.ctrl());
       break;
     default:
-      forward_flow_kernel<T, K, D, GP_KERNEL_EXP><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, c.g->n, kp, c.ctrl());
+      forward_flow_kernel<T, K, D, GP_KERNEL_EXP, MODE><<<grid, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, c.g->n0, first, end, chunk0, kp, c.ctrl());
       break;
   }
   GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+// Cut the graph order into stretches of small and of large batches (see forward_flow_kernel) and launch each.
+template <typename T, int K, int D>
+static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
+  const int L = c.g->n_batches;
+  const int64_t* off = c.g->batch_off;
+  static int64_t in_flight = 0;                 // points the GPU holds at once
+  if (in_flight == 0) {
+    int dev = 0, sms = 0;
+    GP_CUDA_OK(cudaGetDevice(&dev));
+    GP_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    in_flight = (int64_t)sms * GP_FLOW_MIN_CTAS * kCondThreads;
+  }
+  const int64_t large = 2 * in_flight;
+  unsigned long long chunk0 = 0;
+  int b = 0;
+  while (b < L) {
+    auto is_big = [&](int q) {
+      if (c.g->flags & GP_FLAG_FLOW_CARRY) return true;
+      if (c.g->flags & GP_FLAG_FLOW_WEIGHTS) return false;
+      return off[q + 1] - off[q] >= large;
+    };
+    const bool big = is_big(b);
+    int e = b + 1;
+    while (e < L && is_big(e) == big) ++e;
+    // a short run of large batches between small ones is not worth a kernel boundary
+    const int64_t first = off[b], end = off[e];
+    if (big) GP_OK_OR_RETURN((launch_flow_segment<T, K, D, FLOW_CARRY>(c, xi, v, first, end, chunk0)));
+    else GP_OK_OR_RETURN((launch_flow_segment<T, K, D, FLOW_WEIGHTS>(c, xi, v, first, end, chunk0)));
+    chunk0 += (unsigned long long)((end - first + kCondThreads - 1) / kCondThreads);
+    b = e;
+  }
   return GP_OK;
 }
 
