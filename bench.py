@@ -64,6 +64,20 @@ def measured_peaks():
     return HBM_FALLBACK_GBS, "fallback"
 
 
+def profiled_traffic(cid, n, dtype, op):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the op's dominant kernel from the committed
+    `ncu --set full` capture (profiles/r1_traffic.csv: config,n,dtype,op,dram_bytes), or None."""
+    p = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            c = [t.strip() for t in line.split(",")]
+            if len(c) >= 5 and c[0] == str(cid) and c[1] == str(n) and c[2] == dtype and c[3] == op:
+                return float(c[4])
+    return None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -259,6 +273,18 @@ def run_graft(args):
         total_ms = float(t.item())
     ms_per_step = total_ms / args.steps
     value = world * n / (ms_per_step * 1e-3)
+
+    # dominant kernel(s) of each op: CUDA events recorded by the library on the launching stream around the
+    # conditioning kernels (gp_kernel_time_*), over `steps` further steps of the same loop.  Reading an event
+    # synchronises, so this pass is kept out of the region that `value` is computed from.
+    gp.kernel_time_enable(True)
+    kern_ms = {op: [] for op in ops}
+    for s in range(args.steps):
+        for op in ops:
+            do(op)
+            kern_ms[op].append(gp.kernel_time_last())
+    gp.kernel_time_enable(False)
+    kern_ms = {op: float(np.mean(t)) for op, t in kern_ms.items()}
     v_gpu_h = v.cpu().numpy() if rank == 0 else None
 
     # ---- end to end: host (pinned) buffers through the C ABI's *_host calls ------------------------------
@@ -313,18 +339,33 @@ def run_graft(args):
         flop, byt = algorithmic_work(cfg.k, cfg.d, cfg.kind, B, op)
         t_s = op_ms[op] * 1e-3
         t_alu, t_hbm = flop * npts / (alu_peak * 1e12), byt * npts / (hbm * 1e9)
+        k_s = kern_ms[op] * 1e-3
         ops_out[op] = dict(ms=round(op_ms[op], 4), points_per_s=n / t_s, flop_per_point=flop, bytes_per_point=byt,
                            tflops=flop * npts / t_s / 1e12, gbs=byt * npts / t_s / 1e9,
-                           roofline_frac=max(t_alu, t_hbm) / t_s, bound="alu" if t_alu >= t_hbm else "hbm")
-    f = ops_out["forward" if "forward" in ops else ops[0]]
+                           roofline_frac=max(t_alu, t_hbm) / t_s, bound="alu" if t_alu >= t_hbm else "hbm",
+                           kernel_ms=round(kern_ms[op], 4), kernel_roofline_frac=max(t_alu, t_hbm) / k_s)
+    head_op = "forward" if "forward" in ops else ops[0]
+    f = ops_out[head_op]
+    flop, byt = algorithmic_work(cfg.k, cfg.d, cfg.kind, B, head_op)
+    k_s = kern_ms[head_op] * 1e-3
+    k_tflops, k_gbs = flop * npts / k_s / 1e12, byt * npts / k_s / 1e9
+    traffic = profiled_traffic(cfg.cid, n, dtype, head_op)
     if f["bound"] == "alu":
-        roof = dict(bound="alu", achieved=f["tflops"], peak=alu_peak, unit="TFLOP/s", frac=f["tflops"] / alu_peak,
-                    traffic=None, peak_source="nominal non-tensor peak, 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz",
-                    hbm_frac=f["gbs"] / hbm, hbm_peak_source=peak_src)
+        roof = dict(bound="alu", achieved=k_tflops, peak=alu_peak, unit="TFLOP/s", frac=k_tflops / alu_peak,
+                    traffic=traffic, peak_source="nominal non-tensor peak, 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz "
+                    "(DESIGN.md section 7; measured on B200: scalar FFMA 42 TFLOP/s, packed FFMA2 65 TFLOP/s)",
+                    hbm_frac=k_gbs / hbm, hbm_peak_source=peak_src)
     else:
-        roof = dict(bound="hbm", achieved=f["gbs"], peak=hbm, unit="GB/s", frac=f["gbs"] / hbm, traffic=None,
+        roof = dict(bound="hbm", achieved=k_gbs, peak=hbm, unit="GB/s", frac=k_gbs / hbm, traffic=traffic,
                     peak_source=peak_src)
-    roof["kernel"] = "gp_forward (dense head + all batches), CUDA events on the launching stream"
+    roof["kernel"] = {"forward": "forward_flow_kernel (all dataflow launches of gp_forward over the points i >= n0)",
+                      "inverse": "cond_kernel<inverse>", "logdet": "cond_kernel<logdet>",
+                      "vjp": "vjp_geom_kernel + vjp_scatter_kernel"}[head_op]
+    roof["kernel_ms"] = kern_ms[head_op]
+    roof["whole_op_frac"] = f["roofline_frac"]
+    roof["how"] = ("algorithmic flop (bytes) per point x (N - n0) / device time between CUDA events recorded by the "
+                   "library on the launching stream around the kernel(s); whole_op_frac uses the whole gp_forward "
+                   "call (dense head included)")
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,

@@ -151,6 +151,14 @@ const char* gp_status_string(gp_status s);
 
 /* Diagnostics: 1 if (dtype, k, d, kind) has a register-resident specialised kernel, else 0.           */
 int32_t gp_has_specialised(int32_t dtype, int32_t k, int32_t d, int32_t kind);
+/* Kernel timing for the roofline report (bench.py).  While enabled, every op brackets its DOMINANT kernel(s) -
+ * the conditioning kernels over the points i >= n0: the dataflow forward launches, the inverse / logdet kernel,
+ * the VJP geometry + scatter kernels - with CUDA events recorded on the stream they are launched on.
+ * gp_kernel_time_last synchronises on the closing event and returns the device time between the two events of
+ * the most recent op in milliseconds (GP_ERR_INVALID_ARG if nothing was recorded).  Off by default.             */
+void gp_kernel_time_enable(int32_t on);
+gp_status gp_kernel_time_last(double* ms_host);
+
 /* Number of kernels launched by the library in this process so far (for bench.py's gpu_launches).    */
 int64_t gp_launch_count(void);
 

@@ -25,7 +25,8 @@ KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
 
 EXPORTS = ["gp_workspace_bytes", "gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host",
            "gp_inverse_host", "gp_vjp_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
-           "gp_check_errors", "gp_status_string", "gp_has_specialised", "gp_launch_count"]
+           "gp_check_errors", "gp_status_string", "gp_has_specialised", "gp_launch_count", "gp_kernel_time_enable",
+           "gp_kernel_time_last"]
 
 
 class GraphGPError(RuntimeError):
@@ -62,6 +63,10 @@ def lib():
         L.gp_status_string.restype = C.c_char_p
         L.gp_status_string.argtypes = [C.c_int]
         L.gp_launch_count.restype = C.c_int64
+        L.gp_kernel_time_enable.restype = None
+        L.gp_kernel_time_enable.argtypes = [C.c_int32]
+        L.gp_kernel_time_last.restype = C.c_int
+        L.gp_kernel_time_last.argtypes = [C.POINTER(C.c_double)]
         L.gp_has_specialised.restype = C.c_int32
         L.gp_has_specialised.argtypes = [C.c_int32] * 4
         vp, sz = C.c_void_p, C.c_size_t
@@ -90,6 +95,18 @@ def status_string(status: int) -> str:
 
 def launch_count() -> int:
     return int(lib().gp_launch_count())
+
+
+def kernel_time_enable(on: bool) -> None:
+    """Bracket each op's dominant kernel(s) with CUDA events on the launching stream (bench.py's roofline)."""
+    lib().gp_kernel_time_enable(1 if on else 0)
+
+
+def kernel_time_last() -> float:
+    """Device milliseconds of the dominant kernel(s) of the most recent op (synchronises on its closing event)."""
+    ms = C.c_double(0.0)
+    _check(lib().gp_kernel_time_last(C.byref(ms)), "gp_kernel_time_last")
+    return float(ms.value)
 
 
 def has_specialised(dtype: str, k: int, d: int, kind: str) -> bool:

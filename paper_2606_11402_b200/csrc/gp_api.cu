@@ -36,6 +36,22 @@ gp_status side_join(const SideStream* s, cudaStream_t main) {
   return GP_OK;
 }
 
+static std::atomic<int> g_ktime_on{0};
+static cudaEvent_t g_kt0 = nullptr, g_kt1 = nullptr;
+static bool g_kt_recorded = false;
+gp_status ktime_begin(cudaStream_t st) {
+  if (!g_ktime_on.load(std::memory_order_relaxed)) return GP_OK;
+  if (!g_kt0) { GP_CUDA_OK(cudaEventCreate(&g_kt0)); GP_CUDA_OK(cudaEventCreate(&g_kt1)); }
+  GP_CUDA_OK(cudaEventRecord(g_kt0, st));
+  return GP_OK;
+}
+gp_status ktime_end(cudaStream_t st) {
+  if (!g_ktime_on.load(std::memory_order_relaxed) || !g_kt0) return GP_OK;
+  GP_CUDA_OK(cudaEventRecord(g_kt1, st));
+  g_kt_recorded = true;
+  return GP_OK;
+}
+
 static gp_status validate(const gp_graph* g, const gp_kernel* kern) {
   if (!g || !kern) return GP_ERR_INVALID_ARG;
   if (g->n <= 0 || g->n0 < 0 || g->n0 > g->n) return GP_ERR_INVALID_ARG;
@@ -176,6 +192,16 @@ const char* gp_status_string(gp_status s) {
 
 int32_t gp_has_specialised(int32_t dtype, int32_t k, int32_t d, int32_t kind) {
   return has_specialised(dtype, k, d, kind) ? 1 : 0;
+}
+
+void gp_kernel_time_enable(int32_t on) { g_ktime_on.store(on ? 1 : 0, std::memory_order_relaxed); }
+gp_status gp_kernel_time_last(double* ms_host) {
+  if (!ms_host || !g_kt_recorded) return GP_ERR_INVALID_ARG;
+  GP_CUDA_OK(cudaEventSynchronize(g_kt1));
+  float ms = 0.f;
+  GP_CUDA_OK(cudaEventElapsedTime(&ms, g_kt0, g_kt1));
+  *ms_host = (double)ms;
+  return GP_OK;
 }
 
 int64_t gp_launch_count(void) { return (int64_t)g_launches.load(std::memory_order_relaxed); }

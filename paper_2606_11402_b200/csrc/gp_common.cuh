@@ -46,6 +46,7 @@ struct KParams {
   T diag;    // 1 + eps
   T inv_ell;
   T sq;      // sqrt(qscale): the packed fp32 path scales the centred coordinates once instead of every q
+  T inv_diag;  // 1 / (1 + eps)
 };
 
 template <typename T> __host__ inline KParams<T> make_kparams(const gp_kernel& k);
@@ -61,6 +62,7 @@ template <> __host__ inline KParams<float> make_kparams<float>(const gp_kernel& 
   p.qscale = (float)s; p.eps = (float)k.jitter; p.sigma = (float)k.sigma; p.diag = (float)(1.0 + k.jitter);
   p.inv_ell = (float)(1.0 / k.ell);
   p.sq = (float)sqrt(s);
+  p.inv_diag = (float)(1.0 / (1.0 + k.jitter));
   return p;
 }
 template <> __host__ inline KParams<double> make_kparams<double>(const gp_kernel& k) {
@@ -73,6 +75,7 @@ template <> __host__ inline KParams<double> make_kparams<double>(const gp_kernel
   }
   p.qscale = s; p.eps = k.jitter; p.sigma = k.sigma; p.diag = 1.0 + k.jitter; p.inv_ell = 1.0 / k.ell;
   p.sq = sqrt(s);
+  p.inv_diag = 1.0 / (1.0 + k.jitter);
   return p;
 }
 
@@ -225,6 +228,10 @@ struct SideStream {
 gp_status side_stream(SideStream** out);
 gp_status side_fork(const SideStream* s, cudaStream_t main);   // side waits for everything queued on main so far
 gp_status side_join(const SideStream* s, cudaStream_t main);   // main waits for everything queued on side so far
+
+// bench.py's roofline: events around the dominant kernel(s) of the current op, on the launching stream
+gp_status ktime_begin(cudaStream_t st);
+gp_status ktime_end(cudaStream_t st);
 
 // ---- entry points implemented across the .cu files ------------------------------------------------
 // dense head (gp_head.cu)

@@ -30,29 +30,25 @@ template <int K> struct DqStore {
   __device__ __forceinline__ float& scalar(int slot) const { return p1[(size_t)slot * stride]; }
 };
 
-template <int KIND> __device__ __forceinline__ void rho_drho2(f2 q, f2& rho, f2& dr) {
+// gamma = 1 - rho (gp_cond_pk.cuh) and D = ell d rho / d ell for a pair of q's; the MUFU results are shared
+template <int KIND> __device__ __forceinline__ void gamma_drho2(f2 q, f2& gam, f2& dr) {
   const float ln2 = 0.69314718055994530942f;
+  gam = gamma2_from_q<KIND>(q);
   if (KIND == GP_KERNEL_SE) {
     f2 e = make_float2(Math<float>::ex2(-q.x), Math<float>::ex2(-q.y));
-    rho = e;
     dr = mul2(mul2(q, bc(2.0f * ln2)), e);
     return;
   }
   f2 t = make_float2(Math<float>::sqrt_approx(q.x), Math<float>::sqrt_approx(q.y));
   f2 e = make_float2(Math<float>::ex2(-t.x), Math<float>::ex2(-t.y));
   f2 a = mul2(t, bc(ln2));
-  if (KIND == GP_KERNEL_MATERN32) {
-    rho = mul2(add2(a, bc(1.0f)), e);
-    dr = mul2(mul2(a, a), e);
-  } else {
-    rho = e;
-    dr = mul2(a, e);
-  }
+  if (KIND == GP_KERNEL_MATERN32) dr = mul2(mul2(a, a), e);
+  else dr = mul2(a, e);
 }
-template <int KIND> __device__ __forceinline__ void rho_drho1(float q, float& rho, float& dr) {
-  f2 r2, d2;
-  rho_drho2<KIND>(make_float2(q, q), r2, d2);   // the compiler drops the duplicate half
-  rho = r2.x;
+template <int KIND> __device__ __forceinline__ void gamma_drho1(float q, float& gam, float& dr) {
+  f2 g2, d2;
+  gamma_drho2<KIND>(make_float2(q, q), g2, d2);   // the compiler drops the duplicate half
+  gam = g2.x;
   dr = d2.x;
 }
 
@@ -73,11 +69,11 @@ __device__ __forceinline__ void build_joint_grad_pk(const PkCoords<K>& X, const 
       if (D >= 2) { float dy = X.x1[cp].y - c1; q = fmaf(dy, dy, q); }
       if (D >= 3) { float dz = X.x2[cp].y - c2; q = fmaf(dz, dz, q); }
       float r, d;
-      rho_drho1<KIND>(q, r, d);
-      P[pk(cp, c)] = make_float2(kp.diag, r);
+      gamma_drho1<KIND>(q, r, d);
+      P[pk(cp, c)] = make_float2(0.0f, r);
       dq.scalar(cp) = d;
     } else {
-      P[pk(cp, c)] = make_float2(0.0f, kp.diag);
+      P[pk(cp, c)] = make_float2(0.0f, 0.0f);
     }
 #pragma unroll
     for (int rp = cp + 1; rp < H; ++rp) {
@@ -86,7 +82,7 @@ __device__ __forceinline__ void build_joint_grad_pk(const PkCoords<K>& X, const 
       if (D >= 2) { f2 dy = add2(X.x1[rp], bc(-c1)); q = fma2(dy, dy, q); }
       if (D >= 3) { f2 dz = add2(X.x2[rp], bc(-c2)); q = fma2(dz, dz, q); }
       f2 r, d;
-      rho_drho2<KIND>(q, r, d);
+      gamma_drho2<KIND>(q, r, d);
       P[pk(rp, c)] = r;
       dq.full(dq_slot(K, rp, c)) = d;
     }
@@ -94,20 +90,24 @@ __device__ __forceinline__ void build_joint_grad_pk(const PkCoords<K>& X, const 
     if (D >= 2) qs = fmaf(c1, c1, qs);
     if (D >= 3) qs = fmaf(c2, c2, qs);
     float r, d;
-    rho_drho1<KIND>(qs, r, d);
+    gamma_drho1<KIND>(qs, r, d);
     P[pk(H, c)] = make_float2(r, vals[c]);
     dq.scalar(H + c) = d;
   }
-  P[pk(H, K)] = make_float2(kp.diag, 0.0f);
+  P[pk(H, K)] = make_float2(0.0f, 0.0f);
 }
 
-// After factor_joint_pk<K, true>:  W[rp] = (w[2rp], w[2rp+1]) with w = L_cc^-T l,  AL likewise with
-// alpha = L_cc^-T z  (z = the carried values row).
+// After eliminate0_pk and factor_joint_pk<K, true>:  W[rp] = (w[2rp], w[2rp+1]) with w = M_cc^-1 M_ci, AL likewise
+// with alpha = M_cc^-1 v_c.  Rows >= 1 come from the back-substitution on S' = (1 + eps) S (w is scale free; the
+// carried values were not scaled, so alpha picks up the factor 1 + eps), row 0 from the eliminated equation.
 template <int K>
-__device__ __forceinline__ void backsub2_pk(const f2 (&P)[pk_pairs(K)], f2 (&W)[K / 2], f2 (&AL)[K / 2]) {
+__device__ __forceinline__ void backsub2_pk(const f2 (&P)[pk_pairs(K)], const KParams<float>& kp, f2 (&W)[K / 2],
+                                            f2 (&AL)[K / 2]) {
   constexpr int H = K / 2;
+  W[0] = make_float2(0.0f, 0.0f);
+  AL[0] = make_float2(0.0f, 0.0f);
 #pragma unroll
-  for (int j = K - 1; j >= 0; --j) {
+  for (int j = K - 1; j >= 1; --j) {
     const int jp = j / 2, odd = j & 1;
     f2 accw = make_float2(0.0f, 0.0f), acca = make_float2(0.0f, 0.0f);
 #pragma unroll
@@ -125,6 +125,10 @@ __device__ __forceinline__ void backsub2_pk(const f2 (&P)[pk_pairs(K)], f2 (&W)[
     if (odd) { W[jp].y = tw * inv; AL[jp].y = ta * inv; }
     else { W[jp].x = tw * inv; AL[jp].x = ta * inv; }
   }
+#pragma unroll
+  for (int rp = 0; rp < H; ++rp) AL[rp] = mul2(AL[rp], bc(kp.diag));
+  W[0].x = w0_pk<K>(P, W, 1.0f - P[pk(H, 0)].x) * kp.inv_diag;
+  AL[0].x = w0_pk<K>(P, AL, P[pk(H, 0)].y) * kp.inv_diag;
 }
 
 // sum_{r > c} D_rc [ u_r (alpha'_c + two_coef u_c) + alpha'_r u_c ]   with u = (-w, 1), alpha' = (alpha, 0).

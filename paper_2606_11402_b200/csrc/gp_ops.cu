@@ -485,10 +485,11 @@ static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
   GP_OK_OR_RETURN(head_factor(c, nullptr, 0));
   if (spec) GP_OK_OR_RETURN(side_join(side, c.st));
   GP_OK_OR_RETURN(head_forward(c, xi, v, c.rec(), spec));
+  GP_OK_OR_RETURN(ktime_begin(c.st));
   if (flow) {
 #define X(TT, K, D) \
     if constexpr (std::is_same<TT, T>::value) {                    \
-      if (c.g->k == K && c.g->d == D) return launch_flow<T, K, D>(c, xi, v); \
+      if (c.g->k == K && c.g->d == D) { GP_OK_OR_RETURN((launch_flow<T, K, D>(c, xi, v))); return ktime_end(c.st); } \
     }
     GP_SPEC_TABLE(X)
 #undef X
@@ -496,7 +497,7 @@ static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
   const int64_t* off = c.g->batch_off;
   for (int b = 0; b < c.g->n_batches; ++b)
     GP_OK_OR_RETURN((launch_range<T, OPK_FORWARD>(c, spec, v, xi, v, off[b], off[b + 1])));
-  return GP_OK;
+  return ktime_end(c.st);
 }
 
 template <typename T>
@@ -512,7 +513,9 @@ static gp_status inverse_t(const OpCtx& c, const T* v, T* xi) {
   GP_OK_OR_RETURN(head_factor(hc, v, 1, true));
   GP_OK_OR_RETURN(head_inverse_out(hc, xi));
   if (spec) GP_OK_OR_RETURN(pack<T>(c, v));
+  GP_OK_OR_RETURN(ktime_begin(c.st));
   GP_OK_OR_RETURN((launch_range<T, OPK_INVERSE>(c, spec, v, v, xi, c.g->n0, c.g->n)));
+  GP_OK_OR_RETURN(ktime_end(c.st));
   return side_join(side, c.st);
 }
 
@@ -528,7 +531,9 @@ static gp_status logdet_t(const OpCtx& c, double* logdet, double* grad) {
   GP_OK_OR_RETURN(head_factor(hc, nullptr, grad ? 2 * (int)c.g->n0 : 0, true));
   GP_OK_OR_RETURN(head_logdet(hc, &c.ctrl()->acc[0], grad ? &c.ctrl()->acc[2] : nullptr));
   if (spec) GP_OK_OR_RETURN(pack<T>(c, nullptr));
+  GP_OK_OR_RETURN(ktime_begin(c.st));
   GP_OK_OR_RETURN((launch_range<T, OPK_LOGDET>(c, spec, nullptr, nullptr, nullptr, c.g->n0, c.g->n)));
+  GP_OK_OR_RETURN(ktime_end(c.st));
   if (grad) GP_OK_OR_RETURN(run_logdet_grad(c));
   GP_OK_OR_RETURN(side_join(side, c.st));
   finalize_logdet_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), logdet, grad, 2.0 * (double)c.g->n / c.kern->sigma,

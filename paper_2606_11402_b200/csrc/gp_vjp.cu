@@ -144,9 +144,10 @@ __device__ __forceinline__ bool grad_geometry_pk(const Rec<float>* __restrict__ 
     for (int j = 0; j < K; ++j) vals[j] = R[j].v;
     build_joint_grad_pk<K, D, KIND>(X, vals, kp, P, dq);
   }
+  eliminate0_pk<K>(P, kp);
   bool ok = factor_joint_pk<K, true>(P, kp.diag);
-  s = Math<float>::sqrt(P[pk(K / 2, K)].x);
-  backsub2_pk<K>(P, W, AL);
+  s = Math<float>::sqrt(P[pk(K / 2, K)].x * kp.inv_diag);
+  backsub2_pk<K>(P, kp, W, AL);
   return ok;
 }
 
@@ -541,6 +542,7 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
     GP_OK_OR_RETURN(head_factor(hc, nullptr, 2 * (int)n0, true));
   }
   if (spec) GP_OK_OR_RETURN(grad_pack<T>(c, v));
+  GP_OK_OR_RETURN(ktime_begin(c.st));
   bool flowed = false;
   if constexpr (std::is_same<T, float>::value) {
     if (spec && !(c.g->flags & GP_FLAG_PER_BATCH_LAUNCH)) {
@@ -555,6 +557,7 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
     for (int b = c.g->n_batches - 1; b >= 0; --b)
       GP_OK_OR_RETURN((launch_grad_range<T, GRAD_VJP>(c, spec, v, xi, gbar, xibar, off[b], off[b + 1])));
   }
+  GP_OK_OR_RETURN(ktime_end(c.st));
   GP_OK_OR_RETURN(side_join(side, c.st));
   if (n0 > 0) GP_OK_OR_RETURN(head_vjp(c, xi, gbar, xibar, &c.ctrl()->acc[3]));
   finalize_grad_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), 3, 4, 1.0 / c.kern->ell, thetabar);
