@@ -8,7 +8,9 @@
 // needs L[c][j] for all c > j in every lane: one width-L shuffle per (j, c) from the lane that owns row c.
 // Entries above the diagonal inside a slot are computed as harmless finite junk and never read.
 #pragma once
-#include "gp_cond.cuh"
+#include <type_traits>
+
+#include "gp_cond_pk.cuh"
 
 namespace gp {
 
@@ -41,8 +43,14 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
     else if (r == K) R = load_rec<COHERENT>(rec + i);
     X0[s] = R.x0; X1[s] = R.x1; X2[s] = R.x2; V[s] = R.v;
   }
-  // a[s][c], c < cols(s); flattened with a fixed stride so that the indices stay compile-time
+  // a[s][c], c < cols(s): every index is a compile-time constant
   T a[S][K + 1];
+  // fp32 works in the gamma form of gp_cond_pk.cuh: gammas instead of rho, neighbour 0 eliminated analytically
+  // (S' = (1 + eps) x Schur complement), factorisation from column 1.  fp64 keeps the plain form.
+  constexpr bool GAMMA = std::is_same<T, float>::value;
+  constexpr int J0 = GAMMA ? 1 : 0;
+  const T v0 = shfl_grp(V[0], 0, L);
+  T gK = T(0);
 #pragma unroll
   for (int c = 0; c < K; ++c) {
     const int cs = c / L, co = c % L;
@@ -50,6 +58,8 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
     const T c1 = D >= 2 ? shfl_grp(X1[cs], co, L) : T(0);
     const T c2 = D >= 3 ? shfl_grp(X2[cs], co, L) : T(0);
     const T vc = shfl_grp(V[cs], co, L);
+    T gc = T(0);
+    if (GAMMA && c >= 1) gc = shfl_grp(a[cs][0], co, L);        // gamma_c0 from the lane that owns row c
 #pragma unroll
     for (int s = cs; s < S; ++s) {
       const int r = s * L + l;
@@ -57,19 +67,47 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
       T d2 = dx * dx;
       if (D >= 2) { T dy = X1[s] - c1; d2 = Math<T>::fma(dy, dy, d2); }
       if (D >= 3) { T dz = X2[s] - c2; d2 = Math<T>::fma(dz, dz, d2); }
-      const T rho = Math<T>::template rho_from_q<KIND>(d2 * kp.qscale);
       T val = T(0);
-      if (r > c) val = (r == K + 1) ? vc : rho;
-      else if (r == c) val = kp.diag;
+      if constexpr (GAMMA) {
+        const float gam = gamma_from_q<KIND>(d2 * kp.qscale);
+        if (c == 0) {
+          val = gam;                                             // column 0 keeps the gammas g_r
+        } else {
+          const float gr = a[s][0];
+          const float b = kp.eps + gc;
+          if (r > c) {
+            if (r == K + 1) val = fmaf(v0 * kp.inv_diag, b, vc - v0);                 // u_c
+            else val = fmaf(-kp.diag, gam, fmaf(gr, 1.0f - gc, b));                   // S'_rc
+          } else if (r == c) {
+            val = b * (kp.diag + (1.0f - gc));                                        // S'_cc
+          }
+        }
+      } else {
+        const T rho = Math<T>::template rho_from_q<KIND>(d2 * kp.qscale);
+        if (r > c) val = (r == K + 1) ? vc : rho;
+        else if (r == c) val = kp.diag;
+      }
       a[s][c] = val;
     }
   }
+  if constexpr (GAMMA) {
+    gK = shfl_grp(a[K / L][0], K % L, L);
 #pragma unroll
-  for (int s = K / L; s < S; ++s) a[s][K] = (s * L + l == K) ? kp.diag : T(0);
+    for (int s = K / L; s < S; ++s) {
+      const int r = s * L + l;
+      T val = T(0);
+      if (r == K) val = (kp.eps + gK) * (kp.diag + (1.0f - gK));
+      else if (r == K + 1) val = -v0 * (1.0f - gK) * kp.inv_diag;
+      a[s][K] = val;
+    }
+  } else {
+#pragma unroll
+    for (int s = K / L; s < S; ++s) a[s][K] = (s * L + l == K) ? kp.diag : T(0);
+  }
 
   T minpiv = kp.diag;
 #pragma unroll
-  for (int j = 0; j < K; ++j) {
+  for (int j = J0; j < K; ++j) {
     const int js = j / L, jo = j % L;
     const T piv = shfl_grp(a[js][j], jo, L);
     minpiv = Math<T>::fmin(minpiv, piv);
@@ -84,7 +122,7 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
     }
   }
   LgCond<T> out;
-  const T s2 = shfl_grp(a[K / L][K], K % L, L);
+  const T s2 = shfl_grp(a[K / L][K], K % L, L) * (GAMMA ? kp.inv_diag : T(1));
   const T negm = shfl_grp(a[(K + 1) / L][K], (K + 1) % L, L);
   out.self_v = shfl_grp(V[K / L], K % L, L);
   minpiv = Math<T>::fmin(minpiv, s2);

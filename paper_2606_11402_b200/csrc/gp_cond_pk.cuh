@@ -77,7 +77,38 @@ template <int KIND> __device__ __forceinline__ f2 gamma2_from_q(f2 q) {
   p = fma2(a, p, bc(1.0f));
   return blend2(below2(a, 0.125f), mul2(a, p), big);
 }
-template <int KIND> __device__ __forceinline__ float gamma_from_q(float q) { return gamma2_from_q<KIND>(make_float2(q, q)).x; }
+// scalar twin (lane-group kernel): same series, same thresholds
+template <int KIND> __device__ __forceinline__ float gamma_from_q(float q) {
+  const float ln2 = 0.69314718055994530942f;
+  if (KIND == GP_KERNEL_SE) {
+    const float u = q * ln2;
+    const float big = 1.0f - Math<float>::ex2(-q);
+    float p = fmaf(u, 1.0f / 120.0f, -1.0f / 24.0f);
+    p = fmaf(u, p, 1.0f / 6.0f);
+    p = fmaf(u, p, -0.5f);
+    p = fmaf(u, p, 1.0f);
+    return u < 0.125f ? u * p : big;
+  }
+  const float t = Math<float>::sqrt_approx(q);
+  const float a = t * ln2;
+  const float e = Math<float>::ex2(-t);
+  if (KIND == GP_KERNEL_MATERN32) {
+    const float big = fmaf(-(1.0f + a), e, 1.0f);
+    float p = fmaf(a, 1.0f / 5760.0f, -1.0f / 840.0f);
+    p = fmaf(a, p, 1.0f / 144.0f);
+    p = fmaf(a, p, -1.0f / 30.0f);
+    p = fmaf(a, p, 0.125f);
+    p = fmaf(a, p, -1.0f / 3.0f);
+    p = fmaf(a, p, 0.5f);
+    return a < 0.5f ? a * a * p : big;
+  }
+  const float big = 1.0f - e;
+  float p = fmaf(a, 1.0f / 120.0f, -1.0f / 24.0f);
+  p = fmaf(a, p, 1.0f / 6.0f);
+  p = fmaf(a, p, -0.5f);
+  p = fmaf(a, p, 1.0f);
+  return a < 0.125f ? a * p : big;
+}
 
 template <int K> struct PkCoords { f2 x0[K / 2], x1[K / 2], x2[K / 2]; };
 
