@@ -138,6 +138,21 @@ def setup_dist(args):
     return dist, world, rank, local
 
 
+def max_over_ranks(dist, ms, device=None):
+    """Replicas: the step time of the job is the slowest rank's device time (no data-path collective)."""
+    if not dist:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world, n, ms_per_step):
+    """Whole-job throughput of `world` replicas of n points each (weak scaling)."""
+    return world * n / (ms_per_step * 1e-3)
+
+
 def make_workload(cfg, n, dtype, rank):
     """Seeded synthetic inputs: points in user order, xi and v_bar per replica."""
     x = W.make_points(cfg, dtype, n)
@@ -267,12 +282,9 @@ def run_graft(args):
     total_ms = sum(ev[s][0].elapsed_time(ev[s][len(ops)]) for s in range(args.steps))
     op_ms = {op: float(np.mean([ev[s][j].elapsed_time(ev[s][j + 1]) for s in range(args.steps)]))
              for j, op in enumerate(ops)}
-    if dist:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(dist, total_ms, dev)
     ms_per_step = total_ms / args.steps
-    value = world * n / (ms_per_step * 1e-3)
+    value = job_value(world, n, ms_per_step)
 
     # dominant kernel(s) of each op: CUDA events recorded by the library on the launching stream around the
     # conditioning kernels (gp_kernel_time_*), over `steps` further steps of the same loop.  Reading an event
@@ -321,10 +333,7 @@ def run_graft(args):
     e1.record(st)
     torch.cuda.synchronize()
     e2e_ms = e0.elapsed_time(e1) / args.steps
-    if dist:
-        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(dist, e2e_ms, dev)
     # forward xi -> v; inverse v -> xi; logdet -> 8 B; vjp xi, v, v_bar -> xi_bar, theta_bar
     h2d = n * B * sum({"forward": 1, "inverse": 1, "logdet": 0, "vjp": 3}[o] for o in ops)
     d2h = sum({"forward": n * B, "inverse": n * B, "logdet": 8, "vjp": n * B + 16}[o] for o in ops)
@@ -377,7 +386,7 @@ def run_graft(args):
                    "l2": "inputs larger than L2 (nbr %.0f MiB + records %.0f MiB per op)" % (
                        npts * cfg.k * 4 / 2 ** 20, n * 4 * B / 2 ** 20)},
         "ops": ops_out, "roofline": roof,
-        "e2e": {"value": world * n / (e2e_ms * 1e-3), "unit": UNIT, "ms_per_step": e2e_ms,
+        "e2e": {"value": job_value(world, n, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
         "gpu_launches": int(launches), "clocks": clocks,
         "builder": {"wall_s": build_wall, "stage_ms": {k_: float(v_) for k_, v_ in
