@@ -280,16 +280,19 @@ vjp_scatter_kernel(const int32_t* __restrict__ nbr, const float* __restrict__ wb
       acc_ell = (double)(g * q4.y);
     }
   }
-  // block sums (their barriers also order every thread's scatter before thread 0's fence below)
-  const int slot = (int)(blockIdx.x % kAccSlots);
-  block_atomic_add(acc_sigma, &ctrl->slots[0][slot], red);
-  block_atomic_add(acc_ell, &ctrl->slots[1][slot], red);
+  // publish first (the next batch is waiting on it), reduce afterwards: the barrier orders every thread's scatter
+  // before thread 0's fence.  (Summing the CTA's contributions per target in a shared-memory hash table first was
+  // tried: 4.5 ms against 2.95 ms - the table costs more than the L2 atomics it saves.)
+  __syncthreads();
   if (threadIdx.x == 0) {
     long long cnt = end - s_info[0];
     if (cnt > (long long)blockDim.x) cnt = blockDim.x;
     __threadfence();
     atomicAdd(&ctrl->done, (unsigned long long)cnt);
   }
+  const int slot = (int)(blockIdx.x % kAccSlots);
+  block_atomic_add(acc_sigma, &ctrl->slots[0][slot], red);
+  block_atomic_add(acc_ell, &ctrl->slots[1][slot], red);
 }
 
 // ---- generic gradient kernel: triangle in shared memory, any k <= 64, d <= 4 -----------------------------
