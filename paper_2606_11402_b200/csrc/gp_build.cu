@@ -9,7 +9,7 @@
 //              order is itself a valid tree), candidates ranked by (fp64 FMA-free squared
 //              distance, tree index) (R-5).  One thread per query, queries of one warp are
 //              spatial neighbours (heap-order enumeration of each level).
-//   b3 depth   d_i = 1 + max_{j in c(i)} d_j by in-place parallel sweeps until nothing changes.
+//   b3 depth   d_i = 1 + max_{j in c(i)} d_j: the fixed point of PAPER.md:59, reached in one dataflow launch.
 //   b4 sort    stable sort of tree indices by depth (optionally by Morton code inside a depth), remap.
 //
 // Sorting and scanning use CUB (a library primitive on a path that is not the hot path).
@@ -230,18 +230,51 @@ __global__ void max_depth_kernel(const int32_t* __restrict__ depth, int64_t n, u
   if ((threadIdx.x & 31) == 0 && v > 0) atomicMax(out, (unsigned long long)v);
 }
 
-__global__ void depth_sweep_kernel(const int32_t* __restrict__ nbr, int64_t n, int64_t n0, int k,
-                                   int32_t* depth, unsigned long long* changed) {
-  int64_t i = n0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+// d_i = 1 + max_{j in c(i)} d_j.  The paper applies the update to all points in parallel until
+// nothing changes: L sweeps of N k gathers.  The fixed point is unique, so it is reached here in ONE
+// dataflow launch instead: depths start "pending" (-1, head 0), CTAs take chunks of the TREE order through a
+// ticket, and a thread polls its k neighbours (all earlier in tree order, so held by a chunk that has started)
+// until none is pending, then publishes its own depth.  The store sits inside the polling loop, so a neighbour
+// that lives in the same warp makes progress without relying on independent thread scheduling.
+__global__ void depth_init_kernel(int32_t* __restrict__ depth, int64_t n, int64_t n0) {
+  int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) depth[i] = i < n0 ? 0 : -1;
+}
+
+__global__ void __launch_bounds__(256)
+depth_flow_kernel(const int32_t* __restrict__ nbr, int64_t n, int64_t n0, int k, int32_t* depth,
+                  unsigned long long* ticket, unsigned long long* timeout) {
+  __shared__ unsigned long long s_chunk;
+  if (threadIdx.x == 0) s_chunk = atomicAdd(ticket, 1ULL);
+  __syncthreads();
+  const int64_t i = n0 + (int64_t)s_chunk * blockDim.x + threadIdx.x;
   if (i >= n) return;
   const int32_t* row = nbr + (i - n0) * k;
   int32_t m = 0;
-  for (int a = 0; a < k; ++a) {
-    int32_t dj = ((volatile int32_t*)depth)[row[a]];
-    m = dj > m ? dj : m;
+  int a = 0;
+  bool done = false;
+  unsigned spins = 0;
+  const long long t0 = clock64();
+  while (!done) {
+    while (a < k) {
+      int32_t dj;
+      asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(dj) : "l"(depth + row[a]) : "memory");
+      if (dj < 0) break;
+      m = dj > m ? dj : m;
+      ++a;
+    }
+    if (a == k) {
+      asm volatile("st.relaxed.gpu.global.s32 [%0], %1;" ::"l"(depth + i), "r"(m + 1) : "memory");
+      done = true;
+    } else {
+      if (++spins > 4) __nanosleep(spins > 64 ? 200 : 20);
+      if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) {   // watchdog: a bug, never expected
+        atomicAdd(timeout, 1ULL);
+        asm volatile("st.relaxed.gpu.global.s32 [%0], %1;" ::"l"(depth + i), "r"(1) : "memory");
+        done = true;
+      }
+    }
   }
-  int32_t nd = m + 1;
-  if (((volatile int32_t*)depth)[i] != nd) { ((volatile int32_t*)depth)[i] = nd; *changed = 1ULL; }
 }
 
 // ---- b4: depth sort -----------------------------------------------------------------------------------
@@ -422,23 +455,15 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
   GP_CUDA_OK(cudaEventRecord(E.ev[2], st));
 
   // ---- b3: depth fixed point --------------------------------------------------------------
-  GP_CUDA_OK(cudaMemsetAsync(depth_tree, 0, (size_t)n * 4, st));
+  depth_init_kernel<<<nblk(n), 256, 0, st>>>(depth_tree, n, n0);
+  GP_LAUNCH_CHECK();
   int64_t max_depth = 0;
   if (n > n0) {
-    unsigned long long* flag = &ctrl->done;   // builder reuses this slot as its "changed" flag
-    for (int guard = 0; guard < (1 << 22); ++guard) {
-      for (int r = 0; r < 3; ++r) {
-        depth_sweep_kernel<<<nblk(n - n0), 256, 0, st>>>(nbr_tree, n, n0, k, depth_tree, flag);
-        GP_LAUNCH_CHECK();
-      }
-      GP_CUDA_OK(cudaMemsetAsync(flag, 0, 8, st));
-      depth_sweep_kernel<<<nblk(n - n0), 256, 0, st>>>(nbr_tree, n, n0, k, depth_tree, flag);
-      GP_LAUNCH_CHECK();
-      unsigned long long h = 0;
-      GP_CUDA_OK(cudaMemcpyAsync(&h, flag, 8, cudaMemcpyDeviceToHost, st));
-      GP_CUDA_OK(cudaStreamSynchronize(st));
-      if (!h) break;
-    }
+    GP_CUDA_OK(cudaMemsetAsync(&ctrl->ticket, 0, 8, st));
+    GP_CUDA_OK(cudaMemsetAsync(&ctrl->timeout, 0, 8, st));
+    depth_flow_kernel<<<nblk(n - n0), 256, 0, st>>>(nbr_tree, n, n0, k, depth_tree, &ctrl->ticket, &ctrl->timeout);
+    GP_LAUNCH_CHECK();
+    GP_CUDA_OK(cudaMemsetAsync(&ctrl->ticket, 0, 8, st));
     unsigned long long* mx = &ctrl->ticket;
     max_depth_kernel<<<nblk(n), 256, 0, st>>>(depth_tree, n, mx);
     GP_LAUNCH_CHECK();
@@ -446,6 +471,9 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     GP_CUDA_OK(cudaMemcpyAsync(&h, mx, 8, cudaMemcpyDeviceToHost, st));
     GP_CUDA_OK(cudaStreamSynchronize(st));
     max_depth = (int64_t)h;
+    unsigned long long stuck = 0;
+    GP_CUDA_OK(cudaMemcpy(&stuck, &ctrl->timeout, 8, cudaMemcpyDeviceToHost));
+    if (stuck) return GP_ERR_CUDA;                // the depth dataflow's watchdog fired
     if (max_depth > max_batches || max_depth > kMaxBatches) return GP_ERR_INVALID_ARG;
   }
   GP_CUDA_OK(cudaEventRecord(E.ev[3], st));
