@@ -73,30 +73,45 @@ __global__ void head_carry_init_kernel(const T* __restrict__ src, int n0, int mo
 // The whole blocked factorisation in ONE cooperative launch (the per-panel launches of a host loop cost more
 // than the arithmetic: n0 = 1024 is 32 panels, each a strictly serial step).  Per panel two grid barriers:
 //   phase 1  every CTA that owns panel rows factors the 32 x 32 diagonal block (one warp, rows in registers,
-//            pivots broadcast by shuffles), CTA 0 writes it back, then one thread per row solves its panel row;
+//            pivots broadcast by shuffles), CTA 0 writes it back, then one WARP per row solves its panel row;
 //   phase 2  64 x 64 trailing tiles, dealt round-robin to the CTAs.
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
+// 1 / sqrt(x) in full double precision from the fp32 MUFU seed and two Newton steps (2^-22 -> 2^-44 -> 2^-88):
+// a much shorter dependent chain than the library's rsqrt(double), and this chain is what the head waits on.
+__device__ __forceinline__ double rsqrt_fast(double x) {
+  double y = (double)rsqrtf((float)x);
+  double h = 0.5 * x;
+  y = y * fma(-h * y, y, 1.5);
+  y = y * fma(-h * y, y, 1.5);
+  return y;
+}
+
 // Pivot J of the in-register 32 x 32 factorisation (lane r holds row r); a template recursion so that every
 // index into a[] is a compile-time constant (a loop this size is not unrolled reliably -> local memory).
+// The scaled column is broadcast through shared memory (one store per lane, then broadcast loads) rather than
+// by two shuffles per element, and entries above the diagonal are updated too (junk that is never read) so that
+// no select is needed: measured, the shuffle version spent 9 us per 32 x 32 block, 45 % of the whole head.
 template <int J> struct DiagStep {
-  static __device__ __forceinline__ void run(double (&a)[NB], int lane, double* invd, bool& bad) {
+  static __device__ __forceinline__ void run(double (&a)[NB], int lane, double* invd, double* col, bool& bad) {
     double piv = shfl_d(a[J], J);
     bad |= !(piv > 0.0);
-    double inv = rsqrt(piv);                          // CUDA's double rsqrt: 1 ulp
+    double inv = rsqrt_fast(piv);
     double lj = a[J] * inv;                           // lane J: sqrt(piv); lanes > J: L[lane][J]
     a[J] = lj;
     if (lane == J) invd[J] = inv;
+    if (J + 1 < NB) {
+      col[lane] = lj;
+      __syncwarp();
 #pragma unroll
-    for (int c = J + 1; c < NB; ++c) {
-      double lc = shfl_d(lj, c);
-      a[c] = fma(-lj, lane >= c ? lc : 0.0, a[c]);
+      for (int c = J + 1; c < NB; ++c) a[c] = fma(-lj, col[c], a[c]);
+      __syncwarp();
     }
-    DiagStep<J + 1>::run(a, lane, invd, bad);
+    DiagStep<J + 1>::run(a, lane, invd, col, bad);
   }
 };
 template <> struct DiagStep<NB> {
-  static __device__ __forceinline__ void run(double (&)[NB], int, double*, bool&) {}
+  static __device__ __forceinline__ void run(double (&)[NB], int, double*, double*, bool&) {}
 };
 
 __global__ void __launch_bounds__(256)
@@ -104,6 +119,7 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
   cg::grid_group grid = cg::this_grid();
   __shared__ double Ds[NB][NB + 1];
   __shared__ double invd[NB];
+  __shared__ double colbuf[NB];
   __shared__ double Pr[NB][64 + 2];
   __shared__ double Pc[NB][64 + 2];
   const int tid = threadIdx.x, lane = tid & 31;
@@ -113,40 +129,36 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
     const int j1 = j0 + nb;
     const int below = rows_total - j1;
     // ---- phase 1 --------------------------------------------------------------------------------------
-    const int per = (below + G - 1) / G;                  // panel rows per CTA (<= 256 for every size allowed)
-    const int r_begin = j1 + (int)blockIdx.x * per;
-    const int my_rows = max(0, min(per, rows_total - r_begin));
-    if (my_rows > 0 || blockIdx.x == 0) {
+    // panel rows are dealt to WARPS (one row per warp at a time, lane = column): coalesced 256 B row loads, and a
+    // 32-step chain per row instead of one thread grinding through 496 dependent FMAs
+    const int warp = tid >> 5, nwarp = blockDim.x >> 5;
+    const int first_row = j1 + (int)blockIdx.x * nwarp + warp;
+    if ((int)blockIdx.x * nwarp < below || blockIdx.x == 0) {
       if (tid < 32) {
         double a[NB];
 #pragma unroll
         for (int c = 0; c < NB; ++c)
           a[c] = (lane < nb && c <= lane && c < nb) ? A[(size_t)(j0 + lane) * n0 + j0 + c] : (c == lane ? 1.0 : 0.0);
         bool bad = false;
-        DiagStep<0>::run(a, lane, invd, bad);
+        DiagStep<0>::run(a, lane, invd, colbuf, bad);
         if (bad && blockIdx.x == 0 && lane == 0) atomicAdd(&ctrl->n_bad, 1ULL);
 #pragma unroll
         for (int c = 0; c < NB; ++c) {
-          Ds[lane][c] = a[c];
+          Ds[lane][c] = c <= lane ? a[c] : 0.0;
           if (blockIdx.x == 0 && lane < nb && c <= lane) A[(size_t)(j0 + lane) * n0 + j0 + c] = a[c];
         }
       }
       __syncthreads();
-      if (tid < my_rows) {
-        double* arow = A + (size_t)(r_begin + tid) * n0 + j0;
-        double a[NB];
-#pragma unroll
-        for (int c = 0; c < NB; ++c) a[c] = (c < nb) ? arow[c] : 0.0;
+      for (int r = first_row; r < rows_total; r += G * nwarp) {
+        double* arow = A + (size_t)r * n0 + j0;
+        double a = lane < nb ? arow[lane] : 0.0;
 #pragma unroll
         for (int c = 0; c < NB; ++c) {
-          double v = a[c] * invd[c];
-          a[c] = v;
-#pragma unroll
-          for (int c2 = c + 1; c2 < NB; ++c2) a[c2] = fma(-v, Ds[c2][c], a[c2]);
+          const double xc = shfl_d(a, c) * invd[c];
+          if (lane == c) a = xc;
+          else if (lane > c) a = fma(-xc, Ds[lane][c], a);
         }
-#pragma unroll
-        for (int c = 0; c < NB; ++c)
-          if (c < nb) arow[c] = a[c];
+        if (lane < nb) arow[lane] = a;
       }
     }
     grid.sync();
