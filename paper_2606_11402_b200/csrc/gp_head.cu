@@ -120,8 +120,8 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
   __shared__ double Ds[NB][NB + 1];
   __shared__ double invd[NB];
   __shared__ double colbuf[NB];
-  __shared__ double Pr[NB][64 + 2];
-  __shared__ double Pc[NB][64 + 2];
+  __shared__ __align__(16) double Pr[NB][64 + 2];
+  __shared__ __align__(16) double Pc[NB][64 + 2];
   const int tid = threadIdx.x, lane = tid & 31;
   const int G = gridDim.x;
   for (int j0 = 0; j0 < n0; j0 += NB) {
@@ -199,9 +199,13 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
           for (int b_ = 0; b_ < 4; ++b_) acc[a_][b_] = 0.0;
 #pragma unroll 8
         for (int tt = 0; tt < NB; ++tt) {
-          double pr[4], pc[4];
-#pragma unroll
-          for (int a_ = 0; a_ < 4; ++a_) { pr[a_] = Pr[tt][ty * 4 + a_]; pc[a_] = Pc[tt][tx * 4 + a_]; }
+          double pr[4], pc[4];                       // 16 B-aligned: rows are 66 doubles, offsets multiples of 4
+          const double2 r01 = *reinterpret_cast<const double2*>(&Pr[tt][ty * 4]);
+          const double2 r23 = *reinterpret_cast<const double2*>(&Pr[tt][ty * 4 + 2]);
+          const double2 c01 = *reinterpret_cast<const double2*>(&Pc[tt][tx * 4]);
+          const double2 c23 = *reinterpret_cast<const double2*>(&Pc[tt][tx * 4 + 2]);
+          pr[0] = r01.x; pr[1] = r01.y; pr[2] = r23.x; pr[3] = r23.y;
+          pc[0] = c01.x; pc[1] = c01.y; pc[2] = c23.x; pc[3] = c23.y;
 #pragma unroll
           for (int a_ = 0; a_ < 4; ++a_)
 #pragma unroll
