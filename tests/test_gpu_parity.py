@@ -162,6 +162,36 @@ def test_ragged_sizes_all_kernels_fp64(gp, orc, kind, k, d, n0, n):
     assert e["v_rel_max"] <= 1e-9 and e["xi_rel_max"] <= 1e-9 and e["ld_rel"] <= 1e-10, e
 
 
+@pytest.mark.parametrize("kind", ["se", "matern32", "exp"])
+@pytest.mark.parametrize("k,d,n0,n", [(8, 3, 50, 3001), (8, 2, 40, 2600), (16, 3, 64, 4001), (16, 2, 33, 2500),
+                                      (32, 2, 70, 2300), (32, 3, 64, 2100), (5, 3, 5, 700), (7, 2, 9, 900)])
+def test_every_fp32_shape_all_kernels(gp, orc, kind, k, d, n0, n):
+    """Every fp32 kernel shape the library instantiates - packed one-thread-per-point (k = 8, 16; d = 2, 3), lane
+    group (k = 32; d = 2, 3) - and the shared-memory fallback (odd k), each with the three covariance functions,
+    dataflow and per-batch forward.  Jitter 1e-3 and ell = 0.2 on uniform points: a well-conditioned fp32 problem."""
+    import torch
+    x = W.make_points(W.CONFIGS[1], "f32", n)[:, :d].copy()
+    g = orc.build_graph(x.astype(np.float64), k, n0)
+    kd = dict(kind=kind, sigma=1.3, ell=0.2, jitter=1e-3)
+    e = run_all(gp, orc, g, kd, "f32", 1)
+    assert e["v_over_std"] <= F32_V_TOL, e
+    assert e["ld_rel"] <= F32_LOGDET_TOL, e
+    assert e["xi_abs"] <= 2e-3, e
+    e2 = run_all(gp, orc, g, kd, "f32", 1, flags=gp.GP_FLAG_PER_BATCH_LAUNCH)
+    assert e2["v_over_std"] <= F32_V_TOL, e2
+
+
+@pytest.mark.parametrize("k,d", [(16, 2), (8, 2), (16, 3)])
+def test_fp64_lane_group_and_register_shapes(gp, orc, k, d):
+    """fp64: k = 16 runs on the lane-group kernel (d = 2, 3), k = 8 on the one-thread register kernel (d = 2)."""
+    n, n0 = 2777, 48
+    x = W.make_points(W.CONFIGS[1], "f64", n)[:, :d].copy()
+    g = orc.build_graph(x, k, n0)
+    kd = dict(kind="matern32", sigma=0.8, ell=0.15, jitter=1e-6)
+    e = run_all(gp, orc, g, kd, "f64", 1)
+    assert e["v_rel_max"] <= 1e-9 and e["xi_rel_max"] <= 1e-9 and e["ld_rel"] <= 1e-10, e
+
+
 def test_markov_exponential_1d_on_gpu(gp, orc):
     """P-8 on the GPU: d=1, exponential kernel, sorted points, c(i) = {i-1}, no jitter: Vecchia is exact and
     log det = sum log(1 - exp(-2 dx / ell))."""
