@@ -158,3 +158,16 @@ def test_host_variants_match_device_variants(gp, orc):
     xib, tb = gp.gp_vjp(G, K, xi_p.cuda(), v, vb_p.cuda())
     assert np.abs(xib.cpu().numpy() - xib_p.numpy()).max() <= 1e-5 * np.abs(xib_p.numpy()).max()
     assert np.allclose(tb.cpu().numpy(), tb_p.numpy(), rtol=1e-6)
+
+
+@pytest.mark.parametrize("kind", ["se", "matern32", "exp"])
+@pytest.mark.parametrize("k,d,n0,n", [(8, 2, 40, 2600), (16, 2, 33, 2500), (16, 3, 64, 4001), (32, 2, 70, 2300), (7, 2, 9, 900)])
+def test_every_fp32_shape_vjp(gp, orc, kind, k, d, n0, n):
+    """fp32 VJP and log-determinant gradient on every shape: packed two-phase kernels (k = 8, 16; d = 2, 3), and the
+    shared-memory gradient kernel for the shapes without one (k = 32, odd k); dataflow and per-batch variants."""
+    x = W.make_points(W.CONFIGS[1], "f32", n)[:, :d].copy()
+    g = orc.build_graph(x.astype(np.float64), k, n0)
+    kd = dict(kind=kind, sigma=1.3, ell=0.2, jitter=1e-3)
+    for flags in (0, 1):
+        e = run_vjp(gp, orc, g, kd, "f32", 1, flags)
+        assert e["xib"] <= 1e-3 and (e["tb"] <= 1e-3).all() and (e["gld"] <= 1e-3).all(), (flags, e)
