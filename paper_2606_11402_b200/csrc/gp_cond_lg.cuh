@@ -60,6 +60,7 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
     const T vc = shfl_grp(V[cs], co, L);
     T gc = T(0);
     if (GAMMA && c >= 1) gc = shfl_grp(a[cs][0], co, L);        // gamma_c0 from the lane that owns row c
+    constexpr int SV = (K + 1) / L;   // the slot that holds the values row (in lane (K + 1) % L)
 #pragma unroll
     for (int s = cs; s < S; ++s) {
       const int r = s * L + l;
@@ -67,7 +68,9 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
       T d2 = dx * dx;
       if (D >= 2) { T dy = X1[s] - c1; d2 = Math<T>::fma(dy, dy, d2); }
       if (D >= 3) { T dz = X2[s] - c2; d2 = Math<T>::fma(dz, dz, d2); }
-      T val = T(0);
+      // rows of a slot s > cs are all below row c: only slot cs needs the r > c / r == c selects, only slot SV the
+      // values-row select (s and cs are compile-time after unrolling)
+      T val;
       if constexpr (GAMMA) {
         const float gam = gamma_from_q<KIND>(d2 * kp.qscale);
         if (c == 0) {
@@ -75,17 +78,14 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
         } else {
           const float gr = a[s][0];
           const float b = kp.eps + gc;
-          if (r > c) {
-            if (r == K + 1) val = fmaf(v0 * kp.inv_diag, b, vc - v0);                 // u_c
-            else val = fmaf(-kp.diag, gam, fmaf(gr, 1.0f - gc, b));                   // S'_rc
-          } else if (r == c) {
-            val = b * (kp.diag + (1.0f - gc));                                        // S'_cc
-          }
+          val = fmaf(-kp.diag, gam, fmaf(gr, 1.0f - gc, b));                          // S'_rc
+          if (s == SV) val = (r == K + 1) ? fmaf(v0 * kp.inv_diag, b, vc - v0) : val;  // u_c
+          if (s == cs) val = r > c ? val : (r == c ? b * (kp.diag + (1.0f - gc)) : 0.0f);   // S'_cc, above: 0
         }
       } else {
-        const T rho = Math<T>::template rho_from_q<KIND>(d2 * kp.qscale);
-        if (r > c) val = (r == K + 1) ? vc : rho;
-        else if (r == c) val = kp.diag;
+        val = Math<T>::template rho_from_q<KIND>(d2 * kp.qscale);
+        if (s == SV) val = (r == K + 1) ? vc : val;
+        if (s == cs) val = r > c ? val : (r == c ? kp.diag : T(0));
       }
       a[s][c] = val;
     }
