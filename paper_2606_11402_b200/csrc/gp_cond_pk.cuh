@@ -56,26 +56,29 @@ template <int KIND> __device__ __forceinline__ f2 gamma2_from_q(f2 q) {
     p = fma2(u, p, bc(1.0f));
     return blend2(below2(u, 0.125f), mul2(u, p), big);
   }
+  // the series are written in t = a / ln2 (coefficients carry the powers of ln2) so that a itself is never formed
   const f2 t = make_float2(Math<float>::sqrt_approx(q.x), Math<float>::sqrt_approx(q.y));
-  const f2 a = mul2(t, bc(ln2));
   const f2 e = make_float2(Math<float>::ex2(-t.x), Math<float>::ex2(-t.y));
+  constexpr double L1 = 0.69314718055994530942, L2 = L1 * L1, L3 = L2 * L1, L4 = L3 * L1, L5 = L4 * L1, L6 = L5 * L1,
+                   L7 = L6 * L1, L8 = L7 * L1;   // coefficients rounded to fp32 once
+  constexpr float l1 = (float)L1;
   if (KIND == GP_KERNEL_MATERN32) {
-    const f2 big = fma2(neg2(add2(a, bc(1.0f))), e, bc(1.0f));
+    const f2 big = fma2(neg2(fma2(t, bc(l1), bc(1.0f))), e, bc(1.0f));     // 1 - (1 + a) e^-a
     // 1 - (1 + a) e^-a = a^2 (1/2 - a/3 + a^2/8 - a^3/30 + a^4/144 - a^5/840 + a^6/5760 - ...)
-    f2 p = fma2(a, bc(1.0f / 5760.0f), bc(-1.0f / 840.0f));
-    p = fma2(a, p, bc(1.0f / 144.0f));
-    p = fma2(a, p, bc(-1.0f / 30.0f));
-    p = fma2(a, p, bc(0.125f));
-    p = fma2(a, p, bc(-1.0f / 3.0f));
-    p = fma2(a, p, bc(0.5f));
-    return blend2(below2(a, 0.5f), mul2(mul2(a, a), p), big);
+    f2 p = fma2(t, bc((float)(L8 / 5760.0)), bc((float)(-L7 / 840.0)));
+    p = fma2(t, p, bc((float)(L6 / 144.0)));
+    p = fma2(t, p, bc((float)(-L5 / 30.0)));
+    p = fma2(t, p, bc((float)(L4 * 0.125)));
+    p = fma2(t, p, bc((float)(-L3 / 3.0)));
+    p = fma2(t, p, bc((float)(L2 * 0.5)));
+    return blend2(below2(t, 0.5f / l1), mul2(mul2(t, t), p), big);
   }
   const f2 big = add2(bc(1.0f), neg2(e));
-  f2 p = fma2(a, bc(1.0f / 120.0f), bc(-1.0f / 24.0f));
-  p = fma2(a, p, bc(1.0f / 6.0f));
-  p = fma2(a, p, bc(-0.5f));
-  p = fma2(a, p, bc(1.0f));
-  return blend2(below2(a, 0.125f), mul2(a, p), big);
+  f2 p = fma2(t, bc((float)(L5 / 120.0)), bc((float)(-L4 / 24.0)));                        // 1 - e^-a = a (1 - a/2 + a^2/6 - ...)
+  p = fma2(t, p, bc((float)(L3 / 6.0)));
+  p = fma2(t, p, bc((float)(-L2 * 0.5)));
+  p = fma2(t, p, bc(l1));
+  return blend2(below2(t, 0.125f / l1), mul2(t, p), big);
 }
 // scalar twin (lane-group kernel): same series, same thresholds
 template <int KIND> __device__ __forceinline__ float gamma_from_q(float q) {
