@@ -1,5 +1,6 @@
 // Forward / inverse / logdet kernels of the Vecchia conditioning path.
-//   forward  Alg. 1 lines 2-8: one launch per batch, every point of a batch in parallel
+//   forward  Alg. 1 lines 2-8: ticketed dataflow launches over stretches of batches (forward_flow_kernel);
+//            the literal launch per batch is kept behind GP_FLAG_PER_BATCH_LAUNCH and for the lane-group / generic shapes
 //   inverse  PAPER.md:91: every point at once
 //   logdet   PAPER.md:9:  sum_i log s_i^2, fp64 accumulation
 #include <type_traits>

@@ -15,8 +15,10 @@
 // These are the differentials dm = u^T dM [alpha; 0], d(s^2) = u^T dM u of Eq. 2 (R-14); the oracle
 // reaches the same numbers by summing K_bar_ab dK_ab/dtheta over the full joint matrix in the solve form.
 //
-// Batches run in REVERSE order (one launch per batch): a point's cotangent is complete once every later
-// batch has scattered into it, and points of one batch never touch each other's cotangent.
+// Batches run in REVERSE order: a point's cotangent is complete once every later batch has scattered into it, and
+// points of one batch never touch each other's cotangent.  fp32 shapes with a packed kernel: two
+// launches (vjp_geom_kernel, then the ticketed reverse dataflow of vjp_scatter_kernel); every other shape, and
+// GP_FLAG_PER_BATCH_LAUNCH: one grad_kernel launch per batch.
 #include <type_traits>
 
 #include <vector>
