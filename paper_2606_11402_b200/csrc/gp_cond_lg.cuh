@@ -28,12 +28,15 @@ template <typename T, int K, int L> struct LgShape {
 // Result in every lane of the group: m, s (unit sigma), ok, and the point's own value.
 template <typename T> struct LgCond { T m, s, self_v; bool ok; };
 
-template <typename T, int K, int D, int KIND, int L, bool COHERENT>
-__device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ row,
-                                                  int64_t i, int l, const KParams<T>& kp) {
+// Build and factor.  a: the factor (column j >= J0, rows > j), column 0 keeps the gammas in the gamma form; with
+// KEEP_INV the diagonal slot of column j holds 1 / L_jj.  CARRY: the values row is carried (else zeros).
+template <typename T, int K, int D, int KIND, int L, bool COHERENT, bool KEEP_INV, bool CARRY>
+__device__ __forceinline__ void lg_factor(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ row, int64_t i, int l,
+                                          const KParams<T>& kp, T (&a)[LgShape<T, K, L>::S][K + 1],
+                                          T (&V)[LgShape<T, K, L>::S], T& minpiv) {
   using Sh = LgShape<T, K, L>;
   constexpr int S = Sh::S;
-  T X0[S], X1[S], X2[S], V[S];
+  T X0[S], X1[S], X2[S];
 #pragma unroll
   for (int s = 0; s < S; ++s) {
     const int r = s * L + l;
@@ -41,10 +44,8 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
     R.x0 = R.x1 = R.x2 = R.v = T(0);
     if (r < K) R = load_rec<COHERENT>(rec + row[r]);
     else if (r == K) R = load_rec<COHERENT>(rec + i);
-    X0[s] = R.x0; X1[s] = R.x1; X2[s] = R.x2; V[s] = R.v;
+    X0[s] = R.x0; X1[s] = R.x1; X2[s] = R.x2; V[s] = CARRY ? R.v : T(0);
   }
-  // a[s][c], c < cols(s): every index is a compile-time constant
-  T a[S][K + 1];
   // fp32 works in the gamma form of gp_cond_pk.cuh: gammas instead of rho, neighbour 0 eliminated analytically
   // (S' = (1 + eps) x Schur complement), factorisation from column 1.  fp64 keeps the plain form.
   constexpr bool GAMMA = std::is_same<T, float>::value;
@@ -105,7 +106,7 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
     for (int s = K / L; s < S; ++s) a[s][K] = (s * L + l == K) ? kp.diag : T(0);
   }
 
-  T minpiv = kp.diag;
+  minpiv = kp.diag;
 #pragma unroll
   for (int j = J0; j < K; ++j) {
     const int js = j / L, jo = j % L;
@@ -114,6 +115,7 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
     const T inv = Math<T>::rsqrt(piv);
 #pragma unroll
     for (int s = js; s < S; ++s) a[s][j] *= inv;
+    if (KEEP_INV) a[js][j] = (l == jo) ? inv : a[js][j];
 #pragma unroll
     for (int c = j + 1; c <= K; ++c) {
       const T lc = shfl_grp(a[c / L][j], c % L, L);
@@ -121,6 +123,15 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
       for (int s = c / L; s < S; ++s) a[s][c] = Math<T>::fma(-a[s][j], lc, a[s][c]);
     }
   }
+}
+
+template <typename T, int K, int D, int KIND, int L, bool COHERENT>
+__device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ row,
+                                                  int64_t i, int l, const KParams<T>& kp) {
+  constexpr int S = LgShape<T, K, L>::S;
+  constexpr bool GAMMA = std::is_same<T, float>::value;
+  T a[S][K + 1], V[S], minpiv;            // a[s][c], c < cols(s): every index is a compile-time constant
+  lg_factor<T, K, D, KIND, L, COHERENT, false, true>(rec, row, i, l, kp, a, V, minpiv);
   LgCond<T> out;
   const T s2 = shfl_grp(a[K / L][K], K % L, L) * (GAMMA ? kp.inv_diag : T(1));
   const T negm = shfl_grp(a[(K + 1) / L][K], (K + 1) % L, L);
@@ -130,6 +141,58 @@ __device__ __forceinline__ LgCond<T> condition_lg(const Rec<T>* __restrict__ rec
   out.m = -negm;
   out.s = Math<T>::sqrt(s2);
   return out;
+}
+
+// v-independent half for the dataflow forward: every lane ends with the weights of ITS rows (w[s] for row s L + l
+// < K, else 0), s and ok.  Back-substitution  w_j = (l_j - sum_{r > j} L[r][j] w_r) / L_jj : every lane sums over
+// its own rows, the group adds the partial sums with log2 L shuffles, the owner of row j keeps w_j.
+template <typename T> __device__ __forceinline__ T group_sum(T p, int L) {
+  for (int o = L >> 1; o > 0; o >>= 1) p += __shfl_xor_sync(0xffffffffu, p, o, L);
+  return p;
+}
+
+template <typename T, int K, int D, int KIND, int L, bool COHERENT>
+__device__ __forceinline__ void weights_lg(const Rec<T>* __restrict__ rec, const int32_t* __restrict__ row, int64_t i, int l,
+                                           const KParams<T>& kp, T (&w)[LgShape<T, K, L>::S], T& s_out, bool& ok) {
+  constexpr int S = LgShape<T, K, L>::S;
+  constexpr bool GAMMA = std::is_same<T, float>::value;
+  constexpr int J0 = GAMMA ? 1 : 0;
+  T a[S][K + 1], V[S], minpiv;
+  lg_factor<T, K, D, KIND, L, COHERENT, true, false>(rec, row, i, l, kp, a, V, minpiv);
+  const T s2 = shfl_grp(a[K / L][K], K % L, L) * (GAMMA ? kp.inv_diag : T(1));
+  minpiv = Math<T>::fmin(minpiv, s2);
+  ok = (minpiv > T(0)) && (s2 == s2) && (s2 < T(3.0e38));
+  s_out = Math<T>::sqrt(s2);
+#pragma unroll
+  for (int s = 0; s < S; ++s) w[s] = T(0);
+#pragma unroll
+  for (int j = K - 1; j >= J0; --j) {
+    const int js = j / L, jo = j % L;
+    T p = T(0);
+#pragma unroll
+    for (int s = js; s < S; ++s) {
+      // rows of slots > js are all below row j; rows >= K have w = 0; in slot js only rows > j count
+      const T wr = (s == js) ? ((s * L + l > j) ? w[s] : T(0)) : w[s];
+      p = Math<T>::fma(a[s][j], wr, p);
+    }
+    p = group_sum(p, L);
+    const T lj = shfl_grp(a[K / L][j], K % L, L);
+    const T invj = shfl_grp(a[js][j], jo, L);
+    const T wj = (lj - p) * invj;
+    w[js] = (l == jo) ? wj : w[js];
+  }
+  if (GAMMA) {   // row 0 of the eliminated system:  w_0 = ((1 - g_K) - sum_{r >= 1} (1 - g_r) w_r) / (1 + eps)
+    T p = T(0);
+#pragma unroll
+    for (int s = 0; s < S; ++s) {
+      const int r = s * L + l;
+      p = Math<T>::fma(T(1) - a[s][0], (r >= 1 && r < K) ? w[s] : T(0), p);
+    }
+    p = group_sum(p, L);
+    const T gK = shfl_grp(a[K / L][0], K % L, L);
+    const T w0 = ((T(1) - gK) - p) * kp.inv_diag;
+    w[0] = (l == 0) ? w0 : w[0];
+  }
 }
 
 }  // namespace gp

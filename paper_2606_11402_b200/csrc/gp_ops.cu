@@ -4,6 +4,7 @@
 //   inverse  PAPER.md:91: every point at once
 //   logdet   PAPER.md:9:  sum_i log s_i^2, fp64 accumulation
 #include <type_traits>
+#include <vector>
 
 #include "gp_cond_lg.cuh"
 #include "gp_cond_pk.cuh"
@@ -124,6 +125,91 @@ cond_lg_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const 
     }
   }
   if (OP == OPK_LOGDET) block_atomic_add(ld, &ctrl->acc[0], red);
+}
+
+// Dataflow forward for the lane-group shapes (wait-last body only): CTAs take BATCH-ALIGNED chunks of PPB points
+// through a ticket - the groups of one warp then belong to one batch and never wait on each other, so the
+// full-mask shuffles cannot deadlock - weights first, then every lane polls the values of its own rows.
+template <typename T, int K, int D, int KIND, int L>
+__global__ void __launch_bounds__(kCondThreads, 3)
+lg_flow_kernel(Rec<T>* rec, const int32_t* __restrict__ nbr, const T* __restrict__ xi, T* __restrict__ out,
+               const longlong4* __restrict__ tab, int nb, int64_t n0, KParams<T> kp, Control* ctrl) {
+  constexpr int PPB = kCondThreads / L;
+  constexpr int S = LgShape<T, K, L>::S;
+  __shared__ long long s_info[3];
+  __shared__ long long s_ticket;
+  if (threadIdx.x == 0) s_ticket = (long long)atomicAdd(&ctrl->ticket, 1ULL);
+  __syncthreads();
+  {
+    const long long t = s_ticket;
+    for (int q = threadIdx.x; q < nb; q += blockDim.x) {
+      const longlong2 e01 = __ldg(reinterpret_cast<const longlong2*>(tab + q));
+      const longlong2 e23 = __ldg(reinterpret_cast<const longlong2*>(tab + q) + 1);
+      if (e01.x <= t && t < e23.y) {   // {first chunk, rounds << 40 | first point, end point, end chunk} of batch q
+        const long long rounds = e01.y >> 40, first = e01.y & ((1LL << 40) - 1);
+        s_info[0] = first + (t - e01.x) * PPB * rounds;
+        s_info[1] = e23.x;
+        s_info[2] = rounds;
+      }
+    }
+  }
+  __syncthreads();
+  const int l = threadIdx.x % L;
+  const int64_t end = s_info[1];
+  // a ticket covers `rounds` consecutive groups of PPB points of ONE batch (large batches: the ticket and the table
+  // lookup are amortised; small batches: rounds = 1, every point gets its own CTA slot at once)
+  for (int rd = 0; rd < (int)s_info[2]; ++rd) {
+  int64_t i = s_info[0] + (int64_t)rd * PPB + threadIdx.x / L;
+  if (s_info[0] + (int64_t)rd * PPB >= end) break;
+  const bool live = i < end;
+  if (!live) i = end - 1;                     // every lane takes part in the shuffles; the result is dropped
+  const int32_t* row = nbr + (i - n0) * K;
+  T w[S], s;
+  bool ok;
+  weights_lg<T, K, D, KIND, L, true>(rec, row, i, l, kp, w, s, ok);
+  // values of the own rows: all loads in flight first, then poll only what is still pending
+  T vv[S];
+#pragma unroll
+  for (int q = 0; q < S; ++q) vv[q] = (q * L + l < K) ? Pending<T>::load(&rec[row[q * L + l]].v) : T(0);
+  {
+    bool missing = false;
+#pragma unroll
+    for (int q = 0; q < S; ++q) missing |= Pending<T>::is(vv[q]);
+    const long long t0 = clock64();
+    unsigned spins = 0;
+    while (missing) {
+      missing = false;
+#pragma unroll
+      for (int q = 0; q < S; ++q) {
+        if (Pending<T>::is(vv[q])) {
+          vv[q] = Pending<T>::load(&rec[row[q * L + l]].v);
+          missing |= Pending<T>::is(vv[q]);
+        }
+      }
+      if (!missing) break;
+      if (++spins > 8) __nanosleep(spins > 64 ? 256 : 32);
+      if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) {   // watchdog: a bug, never expected
+        atomicAdd(&ctrl->timeout, 1ULL);
+        ok = false;
+        break;
+      }
+    }
+  }
+  T part = T(0);
+#pragma unroll
+  for (int q = 0; q < S; ++q) part = Math<T>::fma(w[q], vv[q], part);
+  const T m = group_sum(part, L);
+  int oki = ok ? 1 : 0;                       // a lane's watchdog may have fired: AND over the group
+  for (int o = L >> 1; o > 0; o >>= 1) oki &= __shfl_xor_sync(0xffffffffu, oki, o, L);
+  ok = oki != 0;
+  if (live && l == 0) {
+    T v = Math<T>::fma(kp.sigma * s, xi[i], m);
+    if (!ok) atomicAdd(&ctrl->n_bad, 1ULL);
+    if (!ok || v != v) v = quiet_nan<T>();
+    out[i] = v;
+    Pending<T>::store(&rec[i].v, v);
+  }
+  }
 }
 
 // ---- dataflow forward: ONE launch for all batches (Alg. 1 lines 2-8) --------------------
@@ -463,6 +549,53 @@ static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
   return GP_OK;
 }
 
+template <typename T, int K, int D, int L>
+static gp_status launch_lg_flow(const OpCtx& c, const T* xi, T* v) {
+  const int nb = c.g->n_batches;
+  if (nb <= 0) return GP_OK;
+  constexpr int PPB = kCondThreads / L;
+  std::vector<int64_t> tab(4 * (size_t)nb);    // per batch {first chunk, first point, end point, end chunk}
+  const int64_t* off = c.g->batch_off;
+  int64_t chunks = 0;
+  static int64_t resident = 0;                 // CTAs the GPU holds at once
+  if (resident == 0) {
+    int dev = 0, sms = 0;
+    GP_CUDA_OK(cudaGetDevice(&dev));
+    GP_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    resident = (int64_t)sms * 3;
+  }
+  for (int b = 0; b < nb; ++b) {
+    const int64_t cnt = off[b + 1] - off[b];
+    int64_t rounds = cnt / (2 * resident * PPB);     // keep at least two waves of tickets per batch
+    rounds = rounds < 1 ? 1 : (rounds > 8 ? 8 : rounds);
+    int64_t nc = (cnt + PPB * rounds - 1) / (PPB * rounds);
+    tab[4 * b + 0] = chunks;
+    tab[4 * b + 1] = (rounds << 40) | off[b];
+    tab[4 * b + 2] = off[b + 1];
+    tab[4 * b + 3] = chunks + nc;
+    chunks += nc;
+  }
+  if (chunks <= 0 || chunks > 0x7fffffffLL) return GP_ERR_UNSUPPORTED;
+  // pageable source: the runtime stages it before returning, so the vector may die afterwards
+  GP_CUDA_OK(cudaMemcpyAsync(c.boff_dev(), tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, c.st));
+  KParams<T> kp = make_kparams<T>(*c.kern);
+  Rec<T>* rec = (Rec<T>*)c.rec();
+  const longlong4* tab_d = (const longlong4*)c.boff_dev();
+  switch (c.kern->kind) {
+    case GP_KERNEL_SE:
+      lg_flow_kernel<T, K, D, GP_KERNEL_SE, L><<<(unsigned)chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, nb, c.g->n0, kp, c.ctrl());
+      break;
+    case GP_KERNEL_MATERN32:
+      lg_flow_kernel<T, K, D, GP_KERNEL_MATERN32, L><<<(unsigned)chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, nb, c.g->n0, kp, c.ctrl());
+      break;
+    default:
+      lg_flow_kernel<T, K, D, GP_KERNEL_EXP, L><<<(unsigned)chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, nb, c.g->n0, kp, c.ctrl());
+      break;
+  }
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
 template <typename T>
 static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
   bool spec = use_spec(c);
@@ -471,6 +604,13 @@ static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
 #define X(TT, K, D) \
     if (std::is_same<TT, T>::value && c.g->k == K && c.g->d == D) flow = true;
     GP_SPEC_TABLE(X)
+#undef X
+    // lane-group shapes: measured, the dataflow launch wins for fp64 k = 16 (config 2: 3.2 -> 2.8 ms) and loses for
+    // fp32 k = 32 (config 4: 30.5 -> 38.5 ms, 651 batches), so k = 32 keeps the launch per batch unless asked
+#define X(TT, K, D, L) \
+    if (std::is_same<TT, T>::value && c.g->k == K && c.g->d == D && (sizeof(T) == 8 || (c.g->flags & GP_FLAG_FLOW_WEIGHTS))) \
+      flow = true;
+    GP_LG_TABLE(X)
 #undef X
   }
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
@@ -493,6 +633,12 @@ static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
       if (c.g->k == K && c.g->d == D) { GP_OK_OR_RETURN((launch_flow<T, K, D>(c, xi, v))); return ktime_end(c.st); } \
     }
     GP_SPEC_TABLE(X)
+#undef X
+#define X(TT, K, D, L) \
+    if constexpr (std::is_same<TT, T>::value) {                    \
+      if (c.g->k == K && c.g->d == D) { GP_OK_OR_RETURN((launch_lg_flow<T, K, D, L>(c, xi, v))); return ktime_end(c.st); } \
+    }
+    GP_LG_TABLE(X)
 #undef X
   }
   const int64_t* off = c.g->batch_off;

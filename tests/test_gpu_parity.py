@@ -240,7 +240,8 @@ def test_argument_errors(gp, orc):
         gp.gp_forward(G2, gp.Kernel("se", 1.0, 0.1, 1e-6), xi)
 
 
-@pytest.mark.parametrize("cid,n,dtype", [(1, 4096, "f64"), (2, 5000, "f32"), (2, 50000, "f32"), (3, 30011, "f32")])
+@pytest.mark.parametrize("cid,n,dtype", [(1, 4096, "f64"), (2, 5000, "f32"), (2, 50000, "f32"), (3, 30011, "f32"),
+                                         (2, 20011, "f64"), (4, 20000, "f32")])   # the last two: lane-group dataflow
 def test_dataflow_forward_equals_per_batch_forward(gp, orc, cid, n, dtype):
     """The single-launch dataflow forward and the literal loop over batches of Alg. 1 apply the
     same weights to the same neighbour values: they agree to rounding (the weights are reached by a different
