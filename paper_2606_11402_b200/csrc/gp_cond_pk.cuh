@@ -45,7 +45,8 @@ __device__ __forceinline__ f2 blend2(f2 w, f2 small, f2 big) { return fma2(w, ad
 // MUFU.EX2 in 1 - rho both stay below about 4e-6 relative to gamma (against 1e-7 / gamma for 1 - rho alone).
 // Measured on config 3 at N = 2^23: max |dv| / std(v) = 1.8e-4 (rho form), 1.05e-4 (threshold 0.17, 3 terms),
 // 7.5e-5 (threshold 0.25, 5 terms), 5.4e-5 (threshold 0.5, 7 terms, series in a), 7.4e-5 (the same series written
-// in t, one packed instruction less per pair: the one kept); the bar is 1e-4.  What is left is the fp32 Cholesky
+// in t, one packed instruction less per pair: the one kept), 1.4e-4 (threshold 0.5 with 6 terms: the dropped term is
+// 5e-6 of gamma at the threshold, and that is already too much); the bar is 1e-4.  What is left is the fp32 Cholesky
 // itself (condition number ~ 1 / eps times the fp32 epsilon).
 template <int KIND> __device__ __forceinline__ f2 gamma2_from_q(f2 q) {
   const float ln2 = 0.69314718055994530942f;
