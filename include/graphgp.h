@@ -10,9 +10,16 @@
  *     paper's bit-reversed k-d tree order stably sorted by depth, head first.
  *   - K_ab = sigma^2 [ rho(|x_a - x_b|) + jitter * delta_ab ]  (relative nugget, R-7).
  *   - "device" = CUDA device memory of the current device; "host" = ordinary host memory.
- *   - Ownership: the caller owns every buffer, including the workspace.  The library allocates
- *     nothing on these calls and keeps no global state.  Calls are asynchronous on `cuda_stream`
- *     (a cudaStream_t passed as void*; NULL = default stream) unless stated otherwise.
+ *   - Ownership: the caller owns every buffer, including the workspace.  The library allocates no
+ *     memory on these calls.  Its only process state: one internal high-priority stream and two events
+ *     per device, created on first use and never destroyed (the dense head runs there beside the bulk
+ *     kernel; everything is joined back into `cuda_stream` before a call returns its work to it), the
+ *     launch counter, and the optional kernel-timing events.  Calls are asynchronous on `cuda_stream`
+ *     (a cudaStream_t passed as void*; NULL = default stream) unless stated otherwise; a workspace must
+ *     not be used by two calls in flight at once.
+ *   - gp_forward and gp_vjp copy a small per-batch table from pageable host memory (staged by the runtime
+ *     before the call returns); gp_forward with the dataflow launch polls device memory and carries a
+ *     watchdog: if it ever fired, gp_check_errors returns GP_ERR_CUDA.
  *   - Errors: return codes only.  Argument errors are synchronous.  A numerical failure (a pivot or
  *     conditional variance that is not positive and finite) writes NaN for that point and increments
  *     a device counter that gp_check_errors() reads.
