@@ -64,18 +64,23 @@ def measured_peaks():
     return HBM_FALLBACK_GBS, "fallback"
 
 
+TRAFFIC_FILES = ("r2_traffic.csv", "r1_traffic.csv")     # newest first
+
+
 def profiled_traffic(cid, n, dtype, op):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the op's dominant kernel from the committed
-    `ncu --set full` capture (profiles/r1_traffic.csv: config,n,dtype,op,dram_bytes), or None."""
-    p = os.path.join(ROOT, "profiles", "r1_traffic.csv")
-    if not os.path.exists(p):
-        return None
-    with open(p) as f:
-        for line in f:
-            c = [t.strip() for t in line.split(",")]
-            if len(c) >= 5 and c[0] == str(cid) and c[1] == str(n) and c[2] == dtype and c[3] == op:
-                return float(c[4])
-    return None
+    """(dram__bytes_read.sum + dram__bytes_write.sum of the op's dominant kernel launches, file it came from) from the
+    committed `ncu --set full` captures (profiles/r*_traffic.csv: config,n,dtype,op,dram_bytes; the .md beside each
+    names the command), or (None, None)."""
+    for name in TRAFFIC_FILES:
+        p = os.path.join(ROOT, "profiles", name)
+        if not os.path.exists(p):
+            continue
+        with open(p) as f:
+            for line in f:
+                c = [t.strip() for t in line.split(",")]
+                if len(c) >= 5 and c[0] == str(cid) and c[1] == str(n) and c[2] == dtype and c[3] == op:
+                    return float(c[4]), "profiles/" + name
+    return None, None
 
 
 class ClockSampler:
@@ -161,9 +166,10 @@ def make_workload(cfg, n, dtype, rank):
     return x, xi, vbar
 
 
-def oracle_sample(cfg, G, xi_h, vbar_h, v_gpu_h, target_s=15.0):
-    """Oracle (as it stands, fp64, OpenMP over the points of a batch) on a PREFIX of the same graph: the first
-    M graph positions are themselves a valid generation graph (every neighbour precedes its point)."""
+def oracle_sample(cfg, G, ops, xi_h, vbar_h, v_gpu_h, target_s=30.0):
+    """Oracle (as it stands, fp64, OpenMP over the points of a batch) on the same graph: ALL N positions when that
+    is about `target_s` seconds of CPU work (configs up to N = 2^24 at k = 16), else a PREFIX of the graph order
+    (the first M positions are themselves a valid generation graph: every neighbour precedes its point)."""
     import oracle as orc
     orc.build()
     OK = orc.Kernel(cfg.kind, cfg.sigma, cfg.ell, cfg.jitter)
@@ -174,29 +180,39 @@ def oracle_sample(cfg, G, xi_h, vbar_h, v_gpu_h, target_s=15.0):
         nbr = G.nbr[:M - n0].cpu().numpy()
         boff = np.unique(np.minimum(G.batch_off, M))
         xi64 = xi_h[:M].astype(np.float64)
+        t = {}
         t0 = time.perf_counter()
         v = orc.forward(xg, OK, xi64, n0=n0, k=k, nbr=nbr, batch_off=boff)
-        t1 = time.perf_counter()
-        orc.inverse(xg, OK, v, n0=n0, k=k, nbr=nbr)
-        t2 = time.perf_counter()
-        orc.logdet(xg, OK, n0=n0, k=k, nbr=nbr)
-        t3 = time.perf_counter()
-        orc.vjp(xg, OK, xi64, v, vbar_h[:M].astype(np.float64), n0=n0, k=k, nbr=nbr, batch_off=boff)
-        t4 = time.perf_counter()
-        return v, dict(forward=t1 - t0, inverse=t2 - t1, logdet=t3 - t2, vjp=t4 - t3)
+        t["forward"] = time.perf_counter() - t0
+        if "inverse" in ops:
+            t0 = time.perf_counter()
+            orc.inverse(xg, OK, v, n0=n0, k=k, nbr=nbr)
+            t["inverse"] = time.perf_counter() - t0
+        if "logdet" in ops:
+            t0 = time.perf_counter()
+            orc.logdet(xg, OK, n0=n0, k=k, nbr=nbr)
+            t["logdet"] = time.perf_counter() - t0
+        if "vjp" in ops:
+            t0 = time.perf_counter()
+            orc.vjp(xg, OK, xi64, v, vbar_h[:M].astype(np.float64), n0=n0, k=k, nbr=nbr, batch_off=boff)
+            t["vjp"] = time.perf_counter() - t0
+        return v, t
 
-    # calibrate on growing prefixes (the dense head and thread start-up dominate small ones), then one run sized
-    # for about target_s seconds of CPU work
-    M = min(n, max(4 * n0, 1 << 16))
-    v, t = run(M)
+    # calibrate on a small prefix (the dense head and thread start-up dominate it: an upper bound per point), then
+    # ONE run: the whole graph if that fits 1.5 x target_s, else the largest power of two that fits target_s
+    M0 = min(n, max(8 * n0, 1 << 17))
+    v, t = run(M0)
     tot = sum(t.values())
-    for _ in range(3):
-        M2 = int(min(n, M * target_s / max(tot, 1e-3)))
-        if M2 < 2 * M:
-            break
-        M = min(n, 1 << int(np.floor(np.log2(M2))))
-        v, t = run(M)
-        tot = sum(t.values())
+    M = M0
+    if M0 < n:
+        per_point = tot / M0
+        if per_point * n <= 1.5 * target_s:
+            M = n
+        else:
+            M = min(n, max(M0, 1 << int(np.floor(np.log2(target_s / per_point)))))
+        if M > M0:
+            v, t = run(M)
+            tot = sum(t.values())
     err = None
     if v_gpu_h is not None:
         err = float(np.abs(v_gpu_h[:M].astype(np.float64) - v).max() / v.std())
@@ -237,7 +253,8 @@ def run_graft(args):
     xi_back = torch.empty_like(xi)
     st = torch.cuda.current_stream()
 
-    ops = [o for o in ("forward", "inverse", "logdet", "vjp") if o in args.ops.split(",")]
+    want = args.ops.split(",") if args.ops else list(cfg.ops)      # default: the ops BASELINE.json lists for the config
+    ops = [o for o in ("forward", "inverse", "logdet", "vjp") if o in want]
     state = {}
     if "forward" not in ops:      # the other ops need a v to work on
         gp.gp_forward(G, K, xi, out=v)
@@ -308,6 +325,7 @@ def run_graft(args):
     in_dev, out_dev = torch.empty_like(xi), torch.empty_like(xi)
     tb_p = torch.empty(2, dtype=torch.float64).pin_memory()
     ld_p = torch.empty(1, dtype=torch.float64).pin_memory()
+    ld_d = torch.empty(1, dtype=torch.float64, device=dev)
     staging = (in_dev, out_dev, torch.empty_like(xi), torch.empty_like(xi), torch.empty(2, dtype=torch.float64, device=dev))
 
     v_p.copy_(v)
@@ -318,7 +336,7 @@ def run_graft(args):
         if "inverse" in ops:
             gp.gp_inverse_host(G, K, v_p, xi2_p, in_dev, out_dev)
         if "logdet" in ops:
-            ld_p.copy_(gp.gp_logdet(G, K), non_blocking=True)
+            gp.gp_logdet_host(G, K, ld_p, ld_d)
         if "vjp" in ops:
             gp.gp_vjp_host(G, K, xi_p, v_p, vbar_p, xib_p, tb_p, staging)
 
@@ -358,15 +376,17 @@ def run_graft(args):
     flop, byt = algorithmic_work(cfg.k, cfg.d, cfg.kind, B, head_op)
     k_s = kern_ms[head_op] * 1e-3
     k_tflops, k_gbs = flop * npts / k_s / 1e12, byt * npts / k_s / 1e9
-    traffic = profiled_traffic(cfg.cid, n, dtype, head_op)
+    traffic, traffic_src = profiled_traffic(cfg.cid, n, dtype, head_op)
+    peak_measured = gp.measure_alu_peak()          # register-resident loops, same process, same clocks (TFLOP/s)
     if f["bound"] == "alu":
         roof = dict(bound="alu", achieved=k_tflops, peak=alu_peak, unit="TFLOP/s", frac=k_tflops / alu_peak,
-                    traffic=traffic, peak_source="nominal non-tensor peak, 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz "
-                    "(DESIGN.md section 7; measured on B200: scalar FFMA 42 TFLOP/s, packed FFMA2 65 TFLOP/s)",
-                    hbm_frac=k_gbs / hbm, hbm_peak_source=peak_src)
+                    traffic=traffic, traffic_source=traffic_src,
+                    peak_source="nominal non-tensor peak, 148 SM x 128 (fp64: 64) lanes x 2 x 1.965 GHz "
+                                "(DESIGN.md section 7); peak_measured = gp_measure_alu_peak in this run",
+                    peak_measured=peak_measured, hbm_frac=k_gbs / hbm, hbm_peak_source=peak_src)
     else:
         roof = dict(bound="hbm", achieved=k_gbs, peak=hbm, unit="GB/s", frac=k_gbs / hbm, traffic=traffic,
-                    peak_source=peak_src)
+                    traffic_source=traffic_src, peak_source=peak_src, peak_measured=peak_measured)
     roof["kernel"] = {"forward": "forward_flow_kernel (all dataflow launches of gp_forward over the points i >= n0)",
                       "inverse": "cond_kernel<inverse>", "logdet": "cond_kernel<logdet>",
                       "vjp": "vjp_geom_kernel + vjp_scatter_kernel"}[head_op]
@@ -392,14 +412,24 @@ def run_graft(args):
         "builder": {"wall_s": build_wall, "stage_ms": {k_: float(v_) for k_, v_ in
                                                        zip(("order", "knn", "depth", "sort"), G.build_ms)}},
     }
+    parity_ok = True
     if not args.no_cpu_baseline:
-        smp = oracle_sample(cfg, G, xi_h, vbar_h, v_gpu_h, target_s=args.cpu_seconds)
+        smp = oracle_sample(cfg, G, ops, xi_h, vbar_h, v_gpu_h, target_s=args.cpu_seconds)
+        what = "all %d graph positions" % n if smp["M"] == n else "first %d graph positions" % smp["M"]
         out["cpu_baseline"] = {"value": smp["M"] / smp["total_s"], "unit": UNIT, "cores": smp["cores"], "kind": "oracle",
-                               "sample": f"first {smp['M']} graph positions of the same graph "
-                                         f"(forward+inverse+logdet+vjp, fp64, {smp['total_s']:.1f} s)",
+                               "sample": f"{what} of the same graph ({'+'.join(smp['seconds'])}, fp64, "
+                                         f"{smp['total_s']:.1f} s)",
                                "seconds": smp["seconds"]}
-        out["parity_on_sample"] = {"max_abs_dv_over_std": smp["v_err_over_std"], "points": smp["M"]}
-    print(json.dumps(out))
+        # north_star: fp64 1e-10 relative to max|v|, fp32 max|dv| <= 1e-4 std(v) (R-16); the oracle's fp64 v
+        # has std ~ max|v| / 5, so the std-relative figure is gated against 5e-10 in fp64
+        tol = 1e-4 if dtype == "f32" else 5e-10
+        parity_ok = smp["v_err_over_std"] is not None and smp["v_err_over_std"] <= tol
+        out["parity_on_sample"] = {"max_abs_dv_over_std": smp["v_err_over_std"], "points": smp["M"], "tolerance": tol,
+                                   "ok": bool(parity_ok)}
+    print(json.dumps(out), flush=True)
+    if not parity_ok:
+        print("bench.py: parity_on_sample exceeds its tolerance: the timing above is not a valid result", file=sys.stderr)
+        sys.exit(3)
 
 
 def run_reference(args):
@@ -421,11 +451,17 @@ def run_reference(args):
     xi = W.make_noise(cfg.cid, M, dtype, "xi").astype(np.float64)
     vbar = W.make_noise(cfg.cid, M, dtype, "vbar").astype(np.float64)
 
+    want = args.ops.split(",") if args.ops else list(cfg.ops)
+    ops = [o for o in ("forward", "inverse", "logdet", "vjp") if o in want]
+
     def step():
         v = orc.forward(g.x, OK, xi, n0=g.n0, k=g.k, nbr=g.nbr, batch_off=g.batch_off)
-        orc.inverse(g.x, OK, v, n0=g.n0, k=g.k, nbr=g.nbr)
-        orc.logdet(g.x, OK, n0=g.n0, k=g.k, nbr=g.nbr)
-        orc.vjp(g.x, OK, xi, v, vbar, n0=g.n0, k=g.k, nbr=g.nbr, batch_off=g.batch_off)
+        if "inverse" in ops:
+            orc.inverse(g.x, OK, v, n0=g.n0, k=g.k, nbr=g.nbr)
+        if "logdet" in ops:
+            orc.logdet(g.x, OK, n0=g.n0, k=g.k, nbr=g.nbr)
+        if "vjp" in ops:
+            orc.vjp(g.x, OK, xi, v, vbar, n0=g.n0, k=g.k, nbr=g.nbr, batch_off=g.batch_off)
 
     for _ in range(args.warmup):
         step()
@@ -435,14 +471,14 @@ def run_reference(args):
     dt = (time.perf_counter() - t0) / args.steps
     value = M / dt
     sample = (f"{M} points drawn by config {cfg.cid}'s recipe (the first {M} user points), graph by the oracle's own "
-              f"order + brute-force neighbours; forward+inverse+logdet+vjp in fp64")
+              f"order + brute-force neighbours; {'+'.join(ops)} in fp64")
     out = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", 1)),
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"config {cfg.cid}: {cfg.name}, bounded sample of {M} points, d={cfg.d}, k={cfg.k}, "
                                f"n0={min(cfg.n0, M)}, {cfg.kind} ell={cfg.ell} jitter={cfg.jitter}",
-                   "step": "forward + inverse + logdet + vjp over the sample"},
+                   "step": " + ".join(ops) + " over the sample"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -459,9 +495,10 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json configuration (1-5); 3 = the headline")
     ap.add_argument("--n", type=int, default=0, help="override the number of points (smaller dry runs)")
     ap.add_argument("--dtype", default="", choices=["", "f32", "f64"])
-    ap.add_argument("--ops", default="forward,inverse,logdet,vjp", help="subset of the step to run (profiling)")
+    ap.add_argument("--ops", default="", help="subset of the step to run (default: the ops BASELINE.json lists for "
+                                              "the configuration; config 3: forward,inverse,logdet,vjp)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the cpu_baseline sample")
+    ap.add_argument("--cpu-seconds", type=float, default=30.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--reference-points", type=int, default=1 << 16)
     args = ap.parse_args()
     if args.impl == "reference":

@@ -111,6 +111,20 @@ def _chunked(n, chunk=1 << 22):
         yield s, min(chunk, n - s)
 
 
+def _for_chunks(n, fill, chunk=1 << 21):
+    """Run fill(start, count) over all chunks; large n uses a thread pool (every element depends on its own
+    counter only, so the result does not depend on the chunking or on the thread count)."""
+    chunks = list(_chunked(n, chunk))
+    if len(chunks) < 4:
+        for s, c in chunks:
+            fill(s, c)
+        return
+    import os
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=min(len(chunks), os.cpu_count() or 1, 32)) as ex:
+        list(ex.map(lambda sc: fill(*sc), chunks))
+
+
 def make_points(cfg: Config, dtype: str, n: int | None = None) -> np.ndarray:
     """Points [n, d] in USER order, values on the grid of `dtype`, returned in that dtype.
 
@@ -122,14 +136,15 @@ def make_points(cfg: Config, dtype: str, n: int | None = None) -> np.ndarray:
     seed = 1000 + cfg.cid
     out = np.empty((n, cfg.d), dtype=dt)
     if cfg.cid in (1, 2):                                   # i.i.d. U[0,1]^3
-        for s, c in _chunked(n):
+        def fill(s, c):
             for j in range(cfg.d):
                 out[s:s + c, j] = uniform(seed, _S_X + j, s, c, dt)
     elif cfg.cid == 3:    # 90 % mixture of 4096 isotropic Gaussians + 10 % uniform background
         ncl = 4096
         cen = np.stack([uniform(seed, _S_CEN + j, 0, ncl, dt) for j in range(3)], axis=1)
         scale = 10.0 ** (-4.0 + 3.0 * uniform(seed, _S_SCALE, 0, ncl, dt))
-        for s, c in _chunked(n):
+
+        def fill(s, c):
             bg = uniform(seed, _S_SEL, s, c, dt) < 0.1
             cl = np.minimum((uniform(seed, _S_CL, s, c, dt) * ncl).astype(np.int64), ncl - 1)
             for j in range(3):
@@ -137,7 +152,7 @@ def make_points(cfg: Config, dtype: str, n: int | None = None) -> np.ndarray:
                 g = normal(seed, _S_G + 2 * j, s, c, dt)
                 out[s:s + c, j] = np.where(bg, u, cen[cl, j] + scale[cl] * g)
     elif cfg.cid == 4:    # radial power law in 2-d: r = U^3, angle uniform
-        for s, c in _chunked(n):
+        def fill(s, c):
             r = uniform(seed, _S_X, s, c, dt) ** 3
             phi = 2.0 * np.pi * uniform(seed, _S_X + 1, s, c, dt)
             out[s:s + c, 0] = r * np.cos(phi)
@@ -146,7 +161,8 @@ def make_points(cfg: Config, dtype: str, n: int | None = None) -> np.ndarray:
         ncl = 1024
         cen = np.stack([uniform(seed, _S_CEN + j, 0, ncl, dt) for j in range(3)], axis=1)
         rad = 10.0 ** (-3.0 + 2.0 * uniform(seed, _S_SCALE, 0, ncl, dt))
-        for s, c in _chunked(n):
+
+        def fill(s, c):
             bg = uniform(seed, _S_SEL, s, c, dt) < 0.5
             cl = np.minimum((uniform(seed, _S_CL, s, c, dt) * ncl).astype(np.int64), ncl - 1)
             g = np.stack([normal(seed, _S_G + 2 * j, s, c, dt) for j in range(3)], axis=1)
@@ -158,6 +174,7 @@ def make_points(cfg: Config, dtype: str, n: int | None = None) -> np.ndarray:
                 out[s:s + c, j] = np.where(bg, u, cen[cl, j] + rr * g[:, j] / gn)
     else:
         raise ValueError(f"unknown config {cfg.cid}")
+    _for_chunks(n, fill)
     return out
 
 
@@ -165,9 +182,11 @@ def make_gaussian_blob(n: int, d: int, dtype: str, seed: int = 1100) -> np.ndarr
     """The paper's own workload shape: points ~ unit Gaussian in d dims."""
     dt = NP_DTYPE[dtype]
     out = np.empty((n, d), dtype=dt)
-    for s, c in _chunked(n):
+
+    def fill(s, c):
         for j in range(d):
             out[s:s + c, j] = normal(seed, _S_G + 2 * j, s, c, dt)
+    _for_chunks(n, fill)
     return out
 
 
@@ -176,6 +195,8 @@ def make_noise(cfg_id: int, n: int, dtype: str, what: str = "xi") -> np.ndarray:
     base = {"xi": 2000, "vbar": 3000}[what]
     dt = NP_DTYPE[dtype]
     out = np.empty(n, dtype=dt)
-    for s, c in _chunked(n):
+
+    def fill(s, c):
         out[s:s + c] = normal(base + cfg_id, _S_NOISE, s, c, dt)
+    _for_chunks(n, fill)
     return out

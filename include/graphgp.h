@@ -11,10 +11,13 @@
  *   - K_ab = sigma^2 [ rho(|x_a - x_b|) + jitter * delta_ab ]  (relative nugget, R-7).
  *   - "device" = CUDA device memory of the current device; "host" = ordinary host memory.
  *   - Ownership: the caller owns every buffer, including the workspace.  The library allocates no
- *     memory on these calls.  Its only process state: one internal high-priority stream and two events
- *     per device, created on first use and never destroyed (the dense head runs there beside the bulk
- *     kernel; everything is joined back into `cuda_stream` before a call returns its work to it), the
- *     launch counter, and the optional kernel-timing events.  Calls are asynchronous on `cuda_stream`
+ *     memory on these calls.  Its only process state, all of it PER DEVICE: one internal high-priority
+ *     stream and two events, created on first use and never destroyed (the dense head runs there beside
+ *     the bulk kernel; everything is joined back into `cuda_stream` before a call returns its work to
+ *     it), the cached SM count, the launch counter, and the optional kernel-timing events.  Calls may
+ *     come from several host threads and on several devices (the side-stream events are taken under a
+ *     per-device mutex; concurrent callers share the one side stream and are serialised on it); the
+ *     kernel-timing diagnostic is meant for one thread.  Calls are asynchronous on `cuda_stream`
  *     (a cudaStream_t passed as void*; NULL = default stream) unless stated otherwise; a workspace must
  *     not be used by two calls in flight at once.
  *   - gp_forward and gp_vjp copy a small per-batch table from pageable host memory (staged by the runtime
@@ -100,7 +103,9 @@ gp_status gp_inverse(const gp_graph* g, const gp_kernel* kern, const void* v, vo
                      size_t ws_bytes, void* cuda_stream);
 
 /* Log-determinant of the Vecchia covariance:  sum_i log s_i^2  (+ log det K_head).
- * logdet_dev: device double[1] (out).  dlogdet_dtheta_dev: device double[2] = d/dsigma, d/dell, or NULL. */
+ * logdet_dev: device double[1] (out).  dlogdet_dtheta_dev: device double[2] = d/dsigma, d/dell, or NULL.
+ * Workspace: gp_workspace_bytes(g, GP_OP_LOGDET) without the gradient; WITH the gradient the call needs the
+ * larger gp_workspace_bytes(g, GP_OP_VJP) (the head carries 2 n0 extra rows), else GP_ERR_WORKSPACE.         */
 gp_status gp_logdet(const gp_graph* g, const gp_kernel* kern, double* logdet_dev, double* dlogdet_dtheta_dev,
                     void* ws, size_t ws_bytes, void* cuda_stream);
 
@@ -119,6 +124,12 @@ gp_status gp_forward_host(const gp_graph* g, const gp_kernel* kern, const void* 
 gp_status gp_inverse_host(const gp_graph* g, const gp_kernel* kern, const void* v_host, void* xi_host,
                           void* in_dev, void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream);
 
+/* gp_logdet with HOST results: the op, then logdet_dev -> logdet_host (and the gradient pair if
+ * dlogdet_dtheta_host != NULL) on `cuda_stream`.  logdet_dev [1] / dlogdet_dtheta_dev [2]: device staging.
+ * Workspace as for gp_logdet.                                                                              */
+gp_status gp_logdet_host(const gp_graph* g, const gp_kernel* kern, double* logdet_host, double* dlogdet_dtheta_host,
+                         double* logdet_dev, double* dlogdet_dtheta_dev, void* ws, size_t ws_bytes, void* cuda_stream);
+
 /* gp_vjp with HOST xi, v, v_bar (in) and xi_bar, theta_bar[2] (out): three [n] host->device copies into the
  * device staging buffers xi_dev, v_dev, v_bar_dev, the VJP, then xi_bar_dev -> xi_bar_host and theta_bar_dev ->
  * theta_bar_host, all on `cuda_stream`.  The caller synchronises the stream before reading the results.  */
@@ -134,8 +145,8 @@ gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_h
  *           tree index)                                                                   (R-5)
  *   depth   d_i = 1 + max_{j in c(i)} d_j by parallel fixed point; head depth 0
  *   sort    graph order = tree order stably sorted by depth; with GP_BUILD_SPATIAL_BATCHES points inside
- *           a batch are additionally ordered by k-d in-order rank (any order inside a batch is legal,
- *           PAPER.md:43) so that neighbouring threads gather neighbouring memory.
+ *           a batch are additionally ordered by Morton code of their coordinates (any order inside a batch is
+ *           legal) so that neighbouring threads gather neighbouring memory.
  * x_user: device [n][d] dtype (in).  Outputs (device unless noted): perm [n] graph position -> user id;
  * x_graph [n][d] dtype; nbr [n-n0][k]; depth [n] (graph order); batch_off_host: HOST int64
  * [max_batches+1]; n_batches: HOST.  Synchronises the stream before returning (batch_off is host data).
@@ -165,6 +176,18 @@ int32_t gp_has_specialised(int32_t dtype, int32_t k, int32_t d, int32_t kind);
  * the most recent op in milliseconds (GP_ERR_INVALID_ARG if nothing was recorded).  Off by default.             */
 void gp_kernel_time_enable(int32_t on);
 gp_status gp_kernel_time_last(double* ms_host);
+
+/* Non-tensor ALU rates of the current device, measured with register-resident loops ("measure
+ * with a register-resident FMA loop under the same clocks").  bench.py prints them beside the NOMINAL peak that
+ * roofline.frac is taken against.  out_host[i], i < min(n_out, GP_PEAK_COUNT), in TFLOP/s (2 flop per fma lane;
+ * MUFU: 1e12 results/s; the two mixed variants count the work of both pipes / of the packed fmas only):
+ *   GP_PEAK_FFMA scalar 3-register fma; GP_PEAK_FFMA_IMM scalar fma with an immediate; GP_PEAK_FFMA2 packed
+ *   fma.rn.f32x2; GP_PEAK_FFMA2_BC packed fma with a broadcast scalar operand (the Cholesky update of the packed
+ *   kernels); GP_PEAK_DFMA; GP_PEAK_MUFU (ex2.approx); GP_PEAK_FFMA2_DFMA and GP_PEAK_FFMA2_MUFU (two pipes at once).
+ * Synchronous (times about 30 short launches with CUDA events on `cuda_stream`).  ws: device scratch >= 256 bytes. */
+enum { GP_PEAK_FFMA = 0, GP_PEAK_FFMA_IMM = 1, GP_PEAK_FFMA2 = 2, GP_PEAK_FFMA2_BC = 3, GP_PEAK_DFMA = 4,
+       GP_PEAK_MUFU = 5, GP_PEAK_FFMA2_DFMA = 6, GP_PEAK_FFMA2_MUFU = 7, GP_PEAK_COUNT = 8 };
+gp_status gp_measure_alu_peak(double* out_host, int32_t n_out, void* ws, size_t ws_bytes, void* cuda_stream);
 
 /* Number of kernels launched by the library in this process so far (for bench.py's gpu_launches).    */
 int64_t gp_launch_count(void);

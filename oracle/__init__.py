@@ -282,6 +282,15 @@ def vjp(x, kern: Kernel, xi, v, vbar, *, n0=0, k=0, nbr=None, rowptr=None, col=N
     return xibar, tb
 
 
+def cond_std(x, kern: Kernel, *, n0=0, k=0, nbr=None, rowptr=None, col=None) -> np.ndarray:
+    """s_i of Eq. 2 for every point (head: diagonal of the dense factor): dv_i / dxi_i."""
+    args, keep, n = _graph_args(x, n0, k, nbr, rowptr, col, None)
+    s = np.empty(n, dtype=np.float64)
+    kc = kern.c()
+    _check(lib().orc_cond_std(*args[:8], C.byref(kc), _p(s, C.c_double)))
+    return s
+
+
 def all_preceding_csr(n: int):
     """c(i) = {0..i-1} for every i (the exact case)."""
     rowptr = np.zeros(n + 1, dtype=np.int64)

@@ -601,6 +601,37 @@ int orc_condition(const double* x, int32_t d, const orc_kernel* kp, int64_t i, c
   return 0;
 }
 
+// Conditional standard deviations s_i = sqrt(K_ii - K_ic K_cc^-1 K_ci) of Eq. 2 for every point:
+// the diagonal of the dense head factor for i < n0 (Alg. 1 line 1: v_head = L0 xi_head, so dv_i/dxi_i = L0_ii),
+// Cond::run for the rest.  Tests use it to express an error of the inverse in units of v (R-16).
+int orc_cond_std(const double* x, int64_t n, int32_t d, int64_t n0, int32_t k, const int32_t* nbr,
+                 const int64_t* rowptr, const int32_t* col, const orc_kernel* kp, double* s_out) {
+  Graph g; g.n = n; g.n0 = n0; g.k = k; g.nbr = nbr; g.rowptr = rowptr; g.col = col;
+  int bad = 0;
+  if (!g.ragged() && n0 > 0) {
+    std::vector<double> L0;
+    if (head_factor<double>(x, d, *kp, n0, L0)) return 3;
+    for (int64_t a = 0; a < n0; ++a) s_out[a] = L0[a * n0 + a];
+  }
+#pragma omp parallel
+  {
+    Cond<double> C;
+#pragma omp for schedule(static)
+    for (int64_t i = g.first(); i < n; ++i) {
+      const int32_t* c; int m;
+      g.row(i, c, m);
+      if (C.run(x, d, *kp, i, c, m)) {
+#pragma omp atomic write
+        bad = 1;
+        s_out[i] = NAN;
+        continue;
+      }
+      s_out[i] = std::sqrt(C.s2);
+    }
+  }
+  return bad ? 3 : 0;
+}
+
 double orc_rho(int32_t kind, double r, double ell) { return rho_of<double>(kind, r, ell); }
 double orc_drho_dell(int32_t kind, double r, double ell) { return drho_dell<double>(kind, r, ell); }
 double orc_d2(const double* a, const double* b, int32_t d) { return d2_canon(a, b, d); }

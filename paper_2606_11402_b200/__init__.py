@@ -24,9 +24,9 @@ GP_BUILD_SPATIAL_BATCHES = 1
 KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
 
 EXPORTS = ["gp_workspace_bytes", "gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host",
-           "gp_inverse_host", "gp_vjp_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
+           "gp_inverse_host", "gp_logdet_host", "gp_vjp_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
            "gp_check_errors", "gp_status_string", "gp_has_specialised", "gp_launch_count", "gp_kernel_time_enable",
-           "gp_kernel_time_last"]
+           "gp_kernel_time_last", "gp_measure_alu_peak"]
 
 
 class GraphGPError(RuntimeError):
@@ -78,12 +78,15 @@ def lib():
         L.gp_forward_host.argtypes = gk + [vp, vp, vp, vp, vp, sz, vp]
         L.gp_inverse_host.argtypes = gk + [vp, vp, vp, vp, vp, sz, vp]
         L.gp_vjp_host.argtypes = gk + [vp] * 11 + [sz, vp]
+        L.gp_logdet_host.argtypes = gk + [vp, vp, vp, vp, vp, sz, vp]
         L.gp_graph_build.argtypes = [vp, C.c_int64, C.c_int32, C.c_int32, C.c_int64, C.c_int32, C.c_int32, vp, vp,
                                      vp, vp, vp, C.c_int32, C.POINTER(C.c_int32), vp, sz, vp]
         L.gp_graph_build_times.argtypes = [vp, vp]
         L.gp_check_errors.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.gp_measure_alu_peak.argtypes = [vp, C.c_int32, vp, sz, vp]
+        L.gp_measure_alu_peak.restype = C.c_int
         for name in ("gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host", "gp_inverse_host",
-                     "gp_vjp_host", "gp_graph_build", "gp_graph_build_times", "gp_check_errors"):
+                     "gp_vjp_host", "gp_logdet_host", "gp_graph_build", "gp_graph_build_times", "gp_check_errors"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -107,6 +110,19 @@ def kernel_time_last() -> float:
     ms = C.c_double(0.0)
     _check(lib().gp_kernel_time_last(C.byref(ms)), "gp_kernel_time_last")
     return float(ms.value)
+
+
+PEAK_NAMES = ("ffma", "ffma_imm", "ffma2", "ffma2_bcast", "dfma", "mufu", "ffma2_dfma", "ffma2_mufu")
+
+
+def measure_alu_peak(stream=None) -> dict:
+    """Non-tensor ALU rates of the current device from register-resident loops (gp_measure_alu_peak), TFLOP/s."""
+    torch = _torch()
+    out = np.zeros(len(PEAK_NAMES), dtype=np.float64)
+    ws = torch.empty(256, dtype=torch.uint8, device="cuda")
+    _check(lib().gp_measure_alu_peak(out.ctypes.data, len(PEAK_NAMES), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
+           "gp_measure_alu_peak")
+    return {k: float(v) for k, v in zip(PEAK_NAMES, out)}
 
 
 def has_specialised(dtype: str, k: int, d: int, kind: str) -> bool:
@@ -161,6 +177,11 @@ class Graph:
         return GP_F64 if self.x.dtype == torch.float64 else GP_F32
 
     def c(self) -> _Graph:
+        torch = _torch()
+        if self.x.device.type != "cuda" or not self.x.is_contiguous() or self.x.dim() != 2:
+            raise ValueError("Graph.x must be a contiguous [n, d] CUDA tensor")
+        if self.nbr.dtype != torch.int32 or not self.nbr.is_contiguous() or self.nbr.device != self.x.device:
+            raise ValueError("Graph.nbr must be a contiguous int32 tensor on the device of Graph.x")
         self.batch_off = np.ascontiguousarray(self.batch_off, dtype=np.int64)
         nb = max(self.batch_off.size - 1, 0)
         return _Graph(self.n, int(self.n0), self.d, self.k, nb, self.dtype_id, int(self.flags), 0,
@@ -202,6 +223,36 @@ def _check(status: int, where: str):
         raise GraphGPError(status, where)
 
 
+def _vec(graph: "Graph", t, name: str, host: bool = False):
+    """Marshalling check: a [n] vector of the graph's dtype, contiguous, on the graph's device (or pinned/host)."""
+    torch = _torch()
+    want = torch.float64 if graph.dtype_id == GP_F64 else torch.float32
+    if not isinstance(t, torch.Tensor):
+        raise TypeError(f"{name}: expected a torch tensor")
+    if t.dtype != want:
+        raise TypeError(f"{name}: dtype {t.dtype} does not match the graph's {want}")
+    if t.numel() != graph.n or not t.is_contiguous():
+        raise ValueError(f"{name}: expected a contiguous vector of {graph.n} elements")
+    if host:
+        if t.device.type != "cpu":
+            raise ValueError(f"{name}: expected a host tensor")
+    elif t.device != graph.x.device:
+        raise ValueError(f"{name}: on {t.device}, the graph is on {graph.x.device}")
+    return t
+
+
+def _f64(t, count: int, name: str, device=None):
+    torch = _torch()
+    if t.dtype != torch.float64 or t.numel() != count or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous float64 tensor of {count} elements")
+    if device is None:
+        if t.device.type != "cpu":
+            raise ValueError(f"{name}: expected a host tensor")
+    elif t.device != device:
+        raise ValueError(f"{name}: on {t.device}, expected {device}")
+    return t
+
+
 def check_errors(ws) -> int:
     """Synchronise, then return the number of points whose conditional was not positive definite."""
     torch = _torch()
@@ -216,7 +267,8 @@ def check_errors(ws) -> int:
 def gp_forward(graph: Graph, kern: Kernel, xi, out=None, stream=None):
     """v = forward(xi): Alg. 1.  xi, v: device [n] in graph order."""
     torch = _torch()
-    v = torch.empty_like(xi) if out is None else out
+    _vec(graph, xi, "xi")
+    v = torch.empty_like(xi) if out is None else _vec(graph, out, "out")
     ws = graph.workspace(GP_OP_FORWARD)
     g, k = graph.c(), kern.c()
     _check(lib().gp_forward(C.byref(g), C.byref(k), xi.data_ptr(), v.data_ptr(), ws.data_ptr(), ws.numel(),
@@ -227,7 +279,8 @@ def gp_forward(graph: Graph, kern: Kernel, xi, out=None, stream=None):
 def gp_inverse(graph: Graph, kern: Kernel, v, out=None, stream=None):
     """xi = inverse(v) (PAPER.md:91)."""
     torch = _torch()
-    xi = torch.empty_like(v) if out is None else out
+    _vec(graph, v, "v")
+    xi = torch.empty_like(v) if out is None else _vec(graph, out, "out")
     ws = graph.workspace(GP_OP_INVERSE)
     g, k = graph.c(), kern.c()
     _check(lib().gp_inverse(C.byref(g), C.byref(k), v.data_ptr(), xi.data_ptr(), ws.data_ptr(), ws.numel(),
@@ -250,6 +303,7 @@ def gp_logdet(graph: Graph, kern: Kernel, grad: bool = False, stream=None):
 def gp_vjp(graph: Graph, kern: Kernel, xi, v, v_bar, stream=None):
     """VJP of gp_forward: returns (xi_bar [n], theta_bar double[2] = d/dsigma, d/dell)."""
     torch = _torch()
+    _vec(graph, xi, "xi"), _vec(graph, v, "v"), _vec(graph, v_bar, "v_bar")
     xi_bar = torch.empty_like(xi)
     tb = torch.empty(2, dtype=torch.float64, device=graph.x.device)
     ws = graph.workspace(GP_OP_VJP)
@@ -261,6 +315,8 @@ def gp_vjp(graph: Graph, kern: Kernel, xi, v, v_bar, stream=None):
 
 def gp_forward_host(graph: Graph, kern: Kernel, xi_host, v_host, in_dev, out_dev, stream=None):
     """End-to-end forward with HOST (pinned) xi / v: H2D copy, forward, D2H copy on one stream."""
+    _vec(graph, xi_host, "xi_host", host=True), _vec(graph, v_host, "v_host", host=True)
+    _vec(graph, in_dev, "in_dev"), _vec(graph, out_dev, "out_dev")
     ws = graph.workspace(GP_OP_FORWARD)
     g, k = graph.c(), kern.c()
     _check(lib().gp_forward_host(C.byref(g), C.byref(k), xi_host.data_ptr(), v_host.data_ptr(), in_dev.data_ptr(),
@@ -270,12 +326,28 @@ def gp_forward_host(graph: Graph, kern: Kernel, xi_host, v_host, in_dev, out_dev
 
 
 def gp_inverse_host(graph: Graph, kern: Kernel, v_host, xi_host, in_dev, out_dev, stream=None):
+    _vec(graph, xi_host, "xi_host", host=True), _vec(graph, v_host, "v_host", host=True)
+    _vec(graph, in_dev, "in_dev"), _vec(graph, out_dev, "out_dev")
     ws = graph.workspace(GP_OP_INVERSE)
     g, k = graph.c(), kern.c()
     _check(lib().gp_inverse_host(C.byref(g), C.byref(k), v_host.data_ptr(), xi_host.data_ptr(), in_dev.data_ptr(),
                                  out_dev.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)),
            "gp_inverse_host")
     return xi_host
+
+
+def gp_logdet_host(graph: Graph, kern: Kernel, logdet_host, logdet_dev, grad_host=None, grad_dev=None, stream=None):
+    """End-to-end logdet: the op, then the device double(s) copied into HOST (pinned) tensors on one stream."""
+    grad = grad_host is not None
+    _f64(logdet_host, 1, "logdet_host"), _f64(logdet_dev, 1, "logdet_dev", graph.x.device)
+    if grad:
+        _f64(grad_host, 2, "grad_host"), _f64(grad_dev, 2, "grad_dev", graph.x.device)
+    ws = graph.workspace(GP_OP_VJP if grad else GP_OP_LOGDET)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_logdet_host(C.byref(g), C.byref(k), logdet_host.data_ptr(), grad_host.data_ptr() if grad else None,
+                                logdet_dev.data_ptr(), grad_dev.data_ptr() if grad else None, ws.data_ptr(), ws.numel(),
+                                _stream_ptr(stream)), "gp_logdet_host")
+    return (logdet_host, grad_host) if grad else logdet_host
 
 
 def gp_vjp_host(graph: Graph, kern: Kernel, xi_host, v_host, vbar_host, xibar_host, theta_bar_host, staging,
@@ -285,6 +357,11 @@ def gp_vjp_host(graph: Graph, kern: Kernel, xi_host, v_host, vbar_host, xibar_ho
     ws = graph.workspace(GP_OP_VJP)
     g, k = graph.c(), kern.c()
     xd, vd, vbd, xbd, tbd = staging
+    for t, nm in ((xi_host, "xi_host"), (v_host, "v_host"), (vbar_host, "vbar_host"), (xibar_host, "xibar_host")):
+        _vec(graph, t, nm, host=True)
+    for t, nm in ((xd, "xi_dev"), (vd, "v_dev"), (vbd, "v_bar_dev"), (xbd, "xi_bar_dev")):
+        _vec(graph, t, nm)
+    _f64(theta_bar_host, 2, "theta_bar_host"), _f64(tbd, 2, "theta_bar_dev", graph.x.device)
     _check(lib().gp_vjp_host(C.byref(g), C.byref(k), xi_host.data_ptr(), v_host.data_ptr(), vbar_host.data_ptr(),
                              xibar_host.data_ptr(), theta_bar_host.data_ptr(), xd.data_ptr(), vd.data_ptr(),
                              vbd.data_ptr(), xbd.data_ptr(), tbd.data_ptr(), ws.data_ptr(), ws.numel(),
@@ -296,6 +373,8 @@ def gp_graph_build(x_user, k: int, n0: int, build_flags: int = GP_BUILD_SPATIAL_
                    stream=None) -> Graph:
     """Build order, preceding-kNN graph, depths and batches on the GPU.  x_user: device [n, d]."""
     torch = _torch()
+    if x_user.device.type != "cuda" or x_user.dim() != 2 or x_user.dtype not in (torch.float32, torch.float64):
+        raise TypeError("gp_graph_build: x_user must be a [n, d] float32/float64 CUDA tensor")
     x_user = x_user.contiguous()
     n, d = int(x_user.shape[0]), int(x_user.shape[1])
     dt = GP_F64 if x_user.dtype == torch.float64 else GP_F32

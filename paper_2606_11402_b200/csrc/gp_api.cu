@@ -2,6 +2,7 @@
 // no allocation, no global state except the launch counter used by bench.py's gpu_launches.
 #include <atomic>
 #include <cstring>
+#include <mutex>
 
 #include "gp_common.cuh"
 
@@ -9,11 +10,30 @@ namespace gp {
 static std::atomic<long long> g_launches{0};
 void count_launch(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+// Per-device state, safe for several host threads: creation and every record + wait pair run under the device's
+// mutex (an event may be re-recorded as soon as the wait on its previous record has been enqueued, so the pair only
+// has to be atomic with respect to other callers).  Work of concurrent callers shares the one side stream of the
+// device and is serialised on it; each caller's fork / join still orders it against that caller's own stream.
+static std::mutex g_dev_mutex[64];
+
+int device_sm_count() {
+  static std::atomic<int> sms[64];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 0;
+  int v = sms[dev].load(std::memory_order_relaxed);
+  if (v == 0) {
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
+    sms[dev].store(v, std::memory_order_relaxed);
+  }
+  return v;
+}
+
 gp_status side_stream(SideStream** out) {
   static SideStream per_dev[64];
   int dev = 0;
   GP_CUDA_OK(cudaGetDevice(&dev));
   if (dev < 0 || dev >= 64) return GP_ERR_CUDA;
+  std::lock_guard<std::mutex> lock(g_dev_mutex[dev]);
   SideStream& s = per_dev[dev];
   if (!s.stream) {
     int lo = 0, hi = 0;
@@ -21,34 +41,47 @@ gp_status side_stream(SideStream** out) {
     GP_CUDA_OK(cudaStreamCreateWithPriority(&s.stream, cudaStreamNonBlocking, hi));
     GP_CUDA_OK(cudaEventCreateWithFlags(&s.fork, cudaEventDisableTiming));
     GP_CUDA_OK(cudaEventCreateWithFlags(&s.join, cudaEventDisableTiming));
+    s.device = dev;
   }
   *out = &s;
   return GP_OK;
 }
 gp_status side_fork(const SideStream* s, cudaStream_t main) {
+  std::lock_guard<std::mutex> lock(g_dev_mutex[s->device]);
   GP_CUDA_OK(cudaEventRecord(s->fork, main));
   GP_CUDA_OK(cudaStreamWaitEvent(s->stream, s->fork, 0));
   return GP_OK;
 }
 gp_status side_join(const SideStream* s, cudaStream_t main) {
+  std::lock_guard<std::mutex> lock(g_dev_mutex[s->device]);
   GP_CUDA_OK(cudaEventRecord(s->join, s->stream));
   GP_CUDA_OK(cudaStreamWaitEvent(main, s->join, 0));
   return GP_OK;
 }
 
+// Kernel timing (a diagnostic for bench.py, off by default): one event pair per device; meant for one host thread.
 static std::atomic<int> g_ktime_on{0};
-static cudaEvent_t g_kt0 = nullptr, g_kt1 = nullptr;
-static bool g_kt_recorded = false;
+struct KTime { cudaEvent_t e0 = nullptr, e1 = nullptr; bool recorded = false; };
+static KTime g_kt[64];
+static KTime* ktime_slot() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+  return &g_kt[dev];
+}
 gp_status ktime_begin(cudaStream_t st) {
   if (!g_ktime_on.load(std::memory_order_relaxed)) return GP_OK;
-  if (!g_kt0) { GP_CUDA_OK(cudaEventCreate(&g_kt0)); GP_CUDA_OK(cudaEventCreate(&g_kt1)); }
-  GP_CUDA_OK(cudaEventRecord(g_kt0, st));
+  KTime* k = ktime_slot();
+  if (!k) return GP_ERR_CUDA;
+  if (!k->e0) { GP_CUDA_OK(cudaEventCreate(&k->e0)); GP_CUDA_OK(cudaEventCreate(&k->e1)); }
+  GP_CUDA_OK(cudaEventRecord(k->e0, st));
   return GP_OK;
 }
 gp_status ktime_end(cudaStream_t st) {
-  if (!g_ktime_on.load(std::memory_order_relaxed) || !g_kt0) return GP_OK;
-  GP_CUDA_OK(cudaEventRecord(g_kt1, st));
-  g_kt_recorded = true;
+  if (!g_ktime_on.load(std::memory_order_relaxed)) return GP_OK;
+  KTime* k = ktime_slot();
+  if (!k || !k->e0) return GP_OK;
+  GP_CUDA_OK(cudaEventRecord(k->e1, st));
+  k->recorded = true;
   return GP_OK;
 }
 
@@ -151,6 +184,17 @@ gp_status gp_inverse_host(const gp_graph* g, const gp_kernel* kern, const void* 
   return GP_OK;
 }
 
+gp_status gp_logdet_host(const gp_graph* g, const gp_kernel* kern, double* logdet_host, double* dlogdet_dtheta_host,
+                         double* logdet_dev, double* dlogdet_dtheta_dev, void* ws, size_t ws_bytes, void* cuda_stream) {
+  if (!g || !logdet_host || !logdet_dev || (dlogdet_dtheta_host && !dlogdet_dtheta_dev)) return GP_ERR_INVALID_ARG;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  GP_OK_OR_RETURN(gp_logdet(g, kern, logdet_dev, dlogdet_dtheta_host ? dlogdet_dtheta_dev : nullptr, ws, ws_bytes, cuda_stream));
+  GP_CUDA_OK(cudaMemcpyAsync(logdet_host, logdet_dev, sizeof(double), cudaMemcpyDeviceToHost, st));
+  if (dlogdet_dtheta_host)
+    GP_CUDA_OK(cudaMemcpyAsync(dlogdet_dtheta_host, dlogdet_dtheta_dev, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  return GP_OK;
+}
+
 gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_host, const void* v_host,
                       const void* v_bar_host, void* xi_bar_host, double* theta_bar_host, void* xi_dev, void* v_dev,
                       void* v_bar_dev, void* xi_bar_dev, double* theta_bar_dev, void* ws, size_t ws_bytes,
@@ -196,10 +240,11 @@ int32_t gp_has_specialised(int32_t dtype, int32_t k, int32_t d, int32_t kind) {
 
 void gp_kernel_time_enable(int32_t on) { g_ktime_on.store(on ? 1 : 0, std::memory_order_relaxed); }
 gp_status gp_kernel_time_last(double* ms_host) {
-  if (!ms_host || !g_kt_recorded) return GP_ERR_INVALID_ARG;
-  GP_CUDA_OK(cudaEventSynchronize(g_kt1));
+  KTime* k = ktime_slot();
+  if (!ms_host || !k || !k->recorded) return GP_ERR_INVALID_ARG;
+  GP_CUDA_OK(cudaEventSynchronize(k->e1));
   float ms = 0.f;
-  GP_CUDA_OK(cudaEventElapsedTime(&ms, g_kt0, g_kt1));
+  GP_CUDA_OK(cudaEventElapsedTime(&ms, k->e0, k->e1));
   *ms_host = (double)ms;
   return GP_OK;
 }

@@ -159,7 +159,7 @@ __device__ __forceinline__ double d2_canon(const double* xi, const T* __restrict
 template <typename T, int KMAX>
 __global__ void __launch_bounds__(128)
 knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int64_t n_threads,
-           int32_t* __restrict__ nbr) {
+           int32_t* __restrict__ nbr, unsigned long long* __restrict__ overflow) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n_threads) return;
   // thread t -> level l, heap position q -> bit-reversed position p -> tree index i: the queries of one
@@ -177,9 +177,13 @@ knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int64_t
   int cnt = 0, worst = 0;
   double wd = 0.0; int32_t wi = -1;
 
+  // the walk pops one entry and pushes at most two children per node, so the stack never holds more than
+  // (tree depth + 1) <= 32 entries for n < 2^31; a push that would not fit is COUNTED (the build then fails)
   struct Ent { int32_t node; double pd2; };
-  Ent stack[40];
+  constexpr int kStack = 40;
+  Ent stack[kStack];
   int sp = 0;
+  bool dropped = false;
   stack[sp++] = {0, 0.0};
   while (sp > 0) {
     Ent e = stack[--sp];
@@ -207,9 +211,10 @@ knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int64_t
     int64_t left = (int64_t)j + ((int64_t)1 << lj), right = (int64_t)j + ((int64_t)2 << lj);
     int64_t near = diff < 0.0 ? left : right, far = diff < 0.0 ? right : left;
     double plane = __dmul_rn(diff, diff);
-    if (far < i && sp < 40) stack[sp++] = {(int32_t)far, plane > e.pd2 ? plane : e.pd2};
-    if (near < i && sp < 40) stack[sp++] = {(int32_t)near, e.pd2};
+    if (far < i) { if (sp < kStack) stack[sp++] = {(int32_t)far, plane > e.pd2 ? plane : e.pd2}; else dropped = true; }
+    if (near < i) { if (sp < kStack) stack[sp++] = {(int32_t)near, e.pd2}; else dropped = true; }
   }
+  if (dropped) atomicAdd(overflow, 1ULL);
   // nearest first (selection sort on (d2, index))
   int32_t* out = nbr + (i - n0) * k;
   for (int a = 0; a < k; ++a) {
@@ -447,9 +452,10 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
   // ---- b2: preceding kNN -----------------------------------------------------------------------------
   if (n > n0) {
     int64_t n_threads = ((int64_t)2 << shape.lam) - 1;
-    if (k <= 16) knn_kernel<T, 16><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree);
-    else if (k <= 32) knn_kernel<T, 32><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree);
-    else knn_kernel<T, 64><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree);
+    unsigned long long* ovf = &ctrl->n_bad;      // zeroed above; read back with the depth watchdog below
+    if (k <= 16) knn_kernel<T, 16><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, ovf);
+    else if (k <= 32) knn_kernel<T, 32><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, ovf);
+    else knn_kernel<T, 64><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, ovf);
     GP_LAUNCH_CHECK();
   }
   GP_CUDA_OK(cudaEventRecord(E.ev[2], st));
@@ -474,6 +480,9 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     unsigned long long stuck = 0;
     GP_CUDA_OK(cudaMemcpy(&stuck, &ctrl->timeout, 8, cudaMemcpyDeviceToHost));
     if (stuck) return GP_ERR_CUDA;                // the depth dataflow's watchdog fired
+    unsigned long long dropped = 0;
+    GP_CUDA_OK(cudaMemcpy(&dropped, &ctrl->n_bad, 8, cudaMemcpyDeviceToHost));
+    if (dropped) return GP_ERR_UNSUPPORTED;       // a kNN walk ran out of stack: the graph would be wrong
     if (max_depth > max_batches || max_depth > kMaxBatches) return GP_ERR_INVALID_ARG;
   }
   GP_CUDA_OK(cudaEventRecord(E.ev[3], st));

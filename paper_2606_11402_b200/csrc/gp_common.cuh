@@ -221,10 +221,13 @@ struct OpCtx {
 // so it runs on a library-internal high-priority stream between a fork event (recorded on the caller's
 // stream) and a join event (waited on by the caller's stream).  One stream and two events per device are
 // created lazily on first use and never destroyed; everything stays ordered with respect to the caller's stream.
+// Thread-safe (per-device mutex around creation and around each record + wait pair).
 struct SideStream {
   cudaStream_t stream = nullptr;
   cudaEvent_t fork = nullptr, join = nullptr;
+  int device = 0;
 };
+int device_sm_count();   // SMs of the current device (cached per device), 0 on error
 gp_status side_stream(SideStream** out);
 gp_status side_fork(const SideStream* s, cudaStream_t main);   // side waits for everything queued on main so far
 gp_status side_join(const SideStream* s, cudaStream_t main);   // main waits for everything queued on side so far

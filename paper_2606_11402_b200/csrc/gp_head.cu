@@ -73,7 +73,8 @@ __global__ void head_carry_init_kernel(const T* __restrict__ src, int n0, int mo
 // The whole blocked factorisation in ONE cooperative launch (the per-panel launches of a host loop cost more
 // than the arithmetic: n0 = 1024 is 32 panels, each a strictly serial step).  Per panel two grid barriers:
 //   phase 1  every CTA that owns panel rows factors the 32 x 32 diagonal block (one warp, rows in registers,
-//            pivots broadcast by shuffles), CTA 0 writes it back, then one WARP per row solves its panel row;
+//            pivots broadcast by shuffles), then one WARP per row solves its panel row; CTA 0 writes the factored
+//            block back after the barrier (the other CTAs read the unfactored one until then);
 //   phase 2  64 x 64 trailing tiles, dealt round-robin to the CTAs.
 __device__ __forceinline__ double shfl_d(double v, int src) { return __shfl_sync(0xffffffffu, v, src); }
 
@@ -143,10 +144,7 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
         DiagStep<0>::run(a, lane, invd, colbuf, bad);
         if (bad && blockIdx.x == 0 && lane == 0) atomicAdd(&ctrl->n_bad, 1ULL);
 #pragma unroll
-        for (int c = 0; c < NB; ++c) {
-          Ds[lane][c] = c <= lane ? a[c] : 0.0;
-          if (blockIdx.x == 0 && lane < nb && c <= lane) A[(size_t)(j0 + lane) * n0 + j0 + c] = a[c];
-        }
+        for (int c = 0; c < NB; ++c) Ds[lane][c] = c <= lane ? a[c] : 0.0;
       }
       __syncthreads();
       for (int r = first_row; r < rows_total; r += G * nwarp) {
@@ -163,6 +161,14 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
     }
     grid.sync();
     // ---- phase 2 --------------------------------------------------------------------------------------
+    // CTA 0 writes the factored diagonal block back only now: during phase 1 the other CTAs were still reading the
+    // unfactored block from A (every CTA factors its own copy), and nothing in this kernel reads it again.
+    if (blockIdx.x == 0) {
+      for (int e = tid; e < NB * NB; e += blockDim.x) {
+        const int r = e / NB, cc = e % NB;
+        if (r < nb && cc <= r) A[(size_t)(j0 + r) * n0 + j0 + cc] = Ds[r][cc];
+      }
+    }
     const int cols = n0 - j1;
     if (cols > 0) {
       const int ntc = (cols + 63) / 64, ntr = (below + 63) / 64;
@@ -256,15 +262,8 @@ gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried, bo
     GP_LAUNCH_CHECK();
   }
   int rows_total = n0 + n_carried;
-  static int grid_ctas = 0;
-  if (grid_ctas == 0) {
-    int dev = 0, sms = 0, per_sm = 0;
-    GP_CUDA_OK(cudaGetDevice(&dev));
-    GP_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    GP_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, head_chol_kernel, 256, 0));
-    if (per_sm < 1) return GP_ERR_CUDA;
-    grid_ctas = sms;                                        // one CTA per SM: all co-resident
-  }
+  const int grid_ctas = device_sm_count();                  // one CTA per SM: all co-resident
+  if (grid_ctas <= 0) return GP_ERR_CUDA;
   int n0_arg = n0;
   Control* ctrl = c.ctrl();
   void* args[] = {(void*)&A, (void*)&n0_arg, (void*)&rows_total, (void*)&ctrl};

@@ -436,11 +436,8 @@ static gp_status launch_generic(const OpCtx& c, const T* vals, const T* in, T* o
   int active = generic_active_threads(k, sizeof(T), false);
   int threads = (active + 31) / 32 * 32;
   size_t smem = (size_t)generic_scratch_elems(k, false) * sizeof(T) * active;
-  static bool attr_set = false;
-  if (!attr_set) {
-    GP_CUDA_OK(cudaFuncSetAttribute(cond_generic_kernel<T, OP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
-    attr_set = true;
-  }
+  // a per-device attribute: set on every launch (cheap next to this kernel) rather than cached per process
+  GP_CUDA_OK(cudaFuncSetAttribute(cond_generic_kernel<T, OP>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
   unsigned grid = (unsigned)((cnt + active - 1) / active);
   KParams<T> kp = make_kparams<T>(*c.kern);
   cond_generic_kernel<T, OP><<<grid, threads, smem, c.st>>>((const T*)c.g->x, vals, c.g->nbr, in, out, start, end,
@@ -520,13 +517,9 @@ template <typename T, int K, int D>
 static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
   const int L = c.g->n_batches;
   const int64_t* off = c.g->batch_off;
-  static int64_t in_flight = 0;                 // points the GPU holds at once
-  if (in_flight == 0) {
-    int dev = 0, sms = 0;
-    GP_CUDA_OK(cudaGetDevice(&dev));
-    GP_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    in_flight = (int64_t)sms * GP_FLOW_MIN_CTAS * kCondThreads;
-  }
+  const int sms = device_sm_count();
+  if (sms <= 0) return GP_ERR_CUDA;
+  const int64_t in_flight = (int64_t)sms * GP_FLOW_MIN_CTAS * kCondThreads;   // points the GPU holds at once
   const int64_t large = 2 * in_flight;
   unsigned long long chunk0 = 0;
   int b = 0;
@@ -539,7 +532,6 @@ static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
     const bool big = is_big(b);
     int e = b + 1;
     while (e < L && is_big(e) == big) ++e;
-    // a short run of large batches between small ones is not worth a kernel boundary
     const int64_t first = off[b], end = off[e];
     if (big) GP_OK_OR_RETURN((launch_flow_segment<T, K, D, FLOW_CARRY>(c, xi, v, first, end, chunk0)));
     else GP_OK_OR_RETURN((launch_flow_segment<T, K, D, FLOW_WEIGHTS>(c, xi, v, first, end, chunk0)));
@@ -557,13 +549,9 @@ static gp_status launch_lg_flow(const OpCtx& c, const T* xi, T* v) {
   std::vector<int64_t> tab(4 * (size_t)nb);    // per batch {first chunk, first point, end point, end chunk}
   const int64_t* off = c.g->batch_off;
   int64_t chunks = 0;
-  static int64_t resident = 0;                 // CTAs the GPU holds at once
-  if (resident == 0) {
-    int dev = 0, sms = 0;
-    GP_CUDA_OK(cudaGetDevice(&dev));
-    GP_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    resident = (int64_t)sms * 3;
-  }
+  const int sms = device_sm_count();
+  if (sms <= 0) return GP_ERR_CUDA;
+  const int64_t resident = (int64_t)sms * 3;   // CTAs the GPU holds at once
   for (int b = 0; b < nb; ++b) {
     const int64_t cnt = off[b + 1] - off[b];
     int64_t rounds = cnt / (2 * resident * PPB);     // keep at least two waves of tickets per batch

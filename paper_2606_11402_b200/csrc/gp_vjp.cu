@@ -268,6 +268,7 @@ vjp_scatter_kernel(const int32_t* __restrict__ nbr, const float* __restrict__ wb
       if (++spins > 16) __nanosleep(32);
       if ((spins & 1023u) == 0 && clock64() - t0 > 8000000000LL) { atomicAdd(&ctrl->timeout, 1ULL); break; }
     }
+    __threadfence();   // acquire side of the done counter: the scatters counted in `d` are visible before gbar is read
   }
   __syncthreads();
   double acc_sigma = 0.0, acc_ell = 0.0;
@@ -401,11 +402,7 @@ static gp_status launch_grad_generic(const OpCtx& c, const T* vals, const T* xi,
   int active = generic_active_threads(k, sizeof(T), true);
   int threads = (active + 31) / 32 * 32;
   size_t smem = (size_t)generic_scratch_elems(k, true) * sizeof(T) * active;
-  static bool attr_set = false;
-  if (!attr_set) {
-    GP_CUDA_OK(cudaFuncSetAttribute(grad_generic_kernel<T, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
-    attr_set = true;
-  }
+  GP_CUDA_OK(cudaFuncSetAttribute(grad_generic_kernel<T, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
   unsigned grid = (unsigned)((cnt + active - 1) / active);
   KParams<T> kp = make_kparams<T>(*c.kern);
   grad_generic_kernel<T, MODE><<<grid, threads, smem, c.st>>>((const T*)c.g->x, vals, c.g->nbr, xi, gbar, xibar, start, end,

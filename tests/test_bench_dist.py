@@ -48,5 +48,5 @@ def test_reference_arm_non_zero_rank_exits_quietly(monkeypatch, capsys):
     import argparse
     import bench
     monkeypatch.setenv("RANK", "1")
-    bench.run_reference(argparse.Namespace(config=1, dtype="", n=0, reference_points=512, steps=1, warmup=0))
+    bench.run_reference(argparse.Namespace(config=1, dtype="", n=0, reference_points=512, steps=1, warmup=0, ops=""))
     assert capsys.readouterr().out == ""

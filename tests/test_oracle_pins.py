@@ -67,6 +67,24 @@ def test_p1_all_preceding_equals_dense_cholesky(orc, kind, sigma, ell, jit):
     assert abs(ld_head - ld_dense) / abs(ld_dense) < 1e-12
 
 
+@pytest.mark.parametrize("kind,sigma,ell,jit", KERNELS)
+def test_p1_conditional_std_is_the_dense_factor_diagonal(orc, kind, sigma, ell, jit):
+    """with c(i) = all preceding points the conditional standard deviations of Eq. 2 are the diagonal
+    of the dense Cholesky factor (LAPACK), through both routes of cond_std (ragged rows; dense head + rows)."""
+    n = 200
+    x = W.make_points(W.CONFIGS[1], "f64", n)
+    kern = orc.Kernel(kind, sigma, ell, jit)
+    Ld = np.diag(np.linalg.cholesky(np_dense_K(x, kind, sigma, ell, jit)))
+    rowptr, col = orc.all_preceding_csr(n)
+    assert rel(orc.cond_std(x, kern, rowptr=rowptr, col=col), Ld) < 1e-10
+    n0 = 60
+    nbr = np.stack([np.arange(i - n0, i, dtype=np.int32) for i in range(n0, n)])   # the n0 points before i
+    s = orc.cond_std(x, kern, n0=n0, k=n0, nbr=nbr)
+    assert rel(s[:n0], Ld[:n0]) < 1e-10
+    # and for a truncated neighbourhood s_i^2 exp-sums to the log-determinant the oracle reports (P-1 pins that one)
+    assert abs(2 * np.log(s).sum() - orc.logdet(x, kern, n0=n0, k=n0, nbr=nbr)) < 1e-8
+
+
 def test_p1_regular_head_plus_rows_equals_ragged(orc):
     """Alg. 1 line 1 (dense head) + per-point rows == every point through Eq. 2 with c(i)={0..i-1} for i<n0."""
     cfg = W.CONFIGS[1]
