@@ -198,21 +198,27 @@ def oracle_sample(cfg, G, ops, xi_h, vbar_h, v_gpu_h, target_s=30.0):
             t["vjp"] = time.perf_counter() - t0
         return v, t
 
-    # calibrate on a small prefix (the dense head and thread start-up dominate it: an upper bound per point), then
-    # ONE run: the whole graph if that fits 1.5 x target_s, else the largest power of two that fits target_s
+    # calibrate on two prefixes (the dense head and thread start-up dominate a small one, so the SLOPE between the two
+    # is the cost per point), then ONE run: the whole graph if that fits 1.5 x target_s, else the largest power of two
     M0 = min(n, max(8 * n0, 1 << 17))
     v, t = run(M0)
     tot = sum(t.values())
     M = M0
     if M0 < n:
-        per_point = tot / M0
-        if per_point * n <= 1.5 * target_s:
-            M = n
-        else:
-            M = min(n, max(M0, 1 << int(np.floor(np.log2(target_s / per_point)))))
-        if M > M0:
-            v, t = run(M)
-            tot = sum(t.values())
+        M1 = min(n, 8 * M0)
+        v, t = run(M1)
+        tot1 = sum(t.values())
+        per_point = max(tot1 - tot, 1e-9) / (M1 - M0)
+        tot, M = tot1, M1
+        if M1 < n:
+            fixed = max(tot1 - per_point * M1, 0.0)
+            if fixed + per_point * n <= 1.5 * target_s:
+                M2 = n
+            else:
+                M2 = min(n, 1 << int(np.floor(np.log2(max(target_s - fixed, 1.0) / per_point))))
+            if M2 > M1:
+                v, t = run(M2)
+                tot, M = sum(t.values()), M2
     err = None
     if v_gpu_h is not None:
         err = float(np.abs(v_gpu_h[:M].astype(np.float64) - v).max() / v.std())
