@@ -151,7 +151,10 @@ gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_h
  * x_graph [n][d] dtype; nbr [n-n0][k]; depth [n] (graph order); batch_off_host: HOST int64
  * [max_batches+1]; n_batches: HOST.  Synchronises the stream before returning (batch_off is host data).
  * Requires n < 2^31.                                                                                   */
-enum { GP_BUILD_SPATIAL_BATCHES = 1 };
+enum { GP_BUILD_SPATIAL_BATCHES = 1,
+       GP_BUILD_RADIUS_CLASSES = 2 /* inside a batch, order first by the class of the neighbourhood radius (distance to
+                                      the farthest of the k neighbours, one class per two octaves), tight first, then
+                                      as GP_BUILD_SPATIAL_BATCHES says.  Optional and off by default. */ };
 gp_status gp_graph_build(const void* x_user, int64_t n, int32_t d, int32_t k, int64_t n0, int32_t dtype,
                          int32_t build_flags, int64_t* perm, void* x_graph, int32_t* nbr, int32_t* depth,
                          int64_t* batch_off_host, int32_t max_batches, int32_t* n_batches, void* ws,

@@ -15,6 +15,7 @@ constexpr int kMaxD = 4;
 constexpr int kCtrlBytes = 2048;
 constexpr int kAccSlots = 64;
 constexpr int kMaxBatches = 1 << 20;
+constexpr int kFlowTickets = 32;   // dataflow forward: launches (stretches of batches) with their own ticket counter
 
 // First kCtrlBytes of every workspace; zeroed by the library at the start of each op.
 struct Control {
@@ -26,6 +27,7 @@ struct Control {
   double build_ms[4];          // graph builder stage times
   unsigned long long pad[4];
   double slots[2][kAccSlots];  // dataflow VJP: per-warp partial sums of sigma_bar / ell_bar, spread to avoid one hot address
+  unsigned long long flow_ticket[kFlowTickets];  // dataflow forward: next 128-point group of each launch
 };
 static_assert(sizeof(Control) <= kCtrlBytes, "control block");
 
@@ -173,11 +175,12 @@ inline size_t dtype_bytes(int dtype) { return dtype == GP_F64 ? 8 : 4; }
 // Workspace layout (byte offsets from ws).  The head is always factored in fp64.
 //   ctrl     Control
 //   boff     dataflow VJP: per batch in reverse order {first chunk, first point, end point, end chunk} (int64 x 4)
+//   gtab     dataflow forward: per 128-point group {first point, end of its batch} (int64 x 2)
 //   head     (n0 + carried) x n0 doubles: factor of K_head/sigma^2 + carried rows (+ n0 doubles for the VJP)
 //   rec      packed records Rec<T>[n]                          (register-resident kernels only)
 //   g        VJP: running cotangent, T[n]
 struct WsLayout {
-  size_t ctrl_off, boff_off, head_off, rec_off, g_off, wbuf_off, total;
+  size_t ctrl_off, boff_off, gtab_off, head_off, rec_off, g_off, wbuf_off, total;
   size_t head_rows;
 };
 inline WsLayout ws_layout(const gp_graph* g, int op) {
@@ -187,6 +190,9 @@ inline WsLayout ws_layout(const gp_graph* g, int op) {
   size_t off = 0;
   w.ctrl_off = off; off += kCtrlBytes;
   w.boff_off = off; off += align_up(4 * ((size_t)g->n_batches + 1) * sizeof(int64_t), 256);
+  // dataflow forward: one {first point, batch end} entry per 128-point group, groups aligned to batches
+  w.gtab_off = off;
+  if (op == GP_OP_FORWARD) off += align_up(((n - n0) / 128 + (size_t)g->n_batches + 1) * 2 * sizeof(int64_t), 256);
   // carried rows: inverse 1 (v_head); gradients 2 n0 (identity -> L^-T, and ell dM/dell -> its L^-1 image)
   size_t carried = (op == GP_OP_INVERSE) ? 1 : (op == GP_OP_VJP ? 2 * n0 : 0);
   w.head_rows = n0 + carried;
@@ -211,6 +217,7 @@ struct OpCtx {
   cudaStream_t st;
   Control* ctrl() const { return (Control*)(ws + lay.ctrl_off); }
   int64_t* boff_dev() const { return (int64_t*)(ws + lay.boff_off); }
+  void* gtab() const { return ws + lay.gtab_off; }
   double* head() const { return (double*)(ws + lay.head_off); }
   void* rec() const { return ws + lay.rec_off; }
   void* gbar() const { return ws + lay.g_off; }
