@@ -362,6 +362,41 @@ def run_graft(args):
     h2d = n * B * sum({"forward": 1, "inverse": 1, "logdet": 0, "vjp": 3}[o] for o in ops)
     d2h = sum({"forward": n * B, "inverse": n * B, "logdet": 8, "vjp": n * B + 16}[o] for o in ops)
 
+    # ---- multi-sample apply: S noise vectors per call on the same graph --------------------
+    multi = None
+    if args.multi > 0 and rank == 0:
+        S = args.multi
+        xi_m = torch.empty((n, S), dtype=tdt, device=dev)
+        for s_ in range(S):
+            xi_m[:, s_] = torch.as_tensor(W.make_noise(cfg.cid + 10 * s_, n, dtype, "xi"), device=dev)
+        v_m = torch.empty_like(xi_m)
+        xi_b = torch.empty_like(xi_m)
+        mt = {}
+        for name, fn in (("forward", lambda: gp.gp_forward_multi(G, K, xi_m, out=v_m)),
+                         ("inverse", lambda: gp.gp_inverse_multi(G, K, v_m, out=xi_b))):
+            for _ in range(max(args.warmup, 1)):
+                fn()
+            torch.cuda.synchronize()
+            m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            m0.record(st)
+            for _ in range(args.steps):
+                fn()
+            m1.record(st)
+            torch.cuda.synchronize()
+            mt[name] = m0.elapsed_time(m1) / args.steps
+        # column 0 of the multi call against the single-sample call on the same noise (xi of this run is sample 0)
+        same = float((v_m[:, 0] - v).abs().max() / v.std()) if "forward" in ops else None
+        back = float((xi_b - xi_m).abs().max())
+        flop1, _ = algorithmic_work(cfg.k, cfg.d, cfg.kind, B, "forward")
+        byt = 4 * cfg.k + cfg.k * cfg.d * B + S * (cfg.k + 2) * B
+        multi = {"samples": S, "forward_ms": mt["forward"], "inverse_ms": mt["inverse"],
+                 "forward_point_samples_per_s": n * S / (mt["forward"] * 1e-3),
+                 "inverse_point_samples_per_s": n * S / (mt["inverse"] * 1e-3),
+                 "bytes_per_point": byt, "flop_per_point": flop1 + 2 * cfg.k * S,
+                 "forward_gbs": byt * (n - G.n0) / (mt["forward"] * 1e-3) / 1e9,
+                 "max_abs_dv_over_std_vs_single_call": same, "max_abs_inverse_of_forward_minus_xi": back}
+        del xi_m, v_m, xi_b
+
     if rank != 0:
         return
     hbm, peak_src = measured_peaks()
@@ -418,6 +453,8 @@ def run_graft(args):
         "builder": {"wall_s": build_wall, "stage_ms": {k_: float(v_) for k_, v_ in
                                                        zip(("order", "knn", "depth", "sort"), G.build_ms)}},
     }
+    if multi is not None:
+        out["multi"] = multi
     parity_ok = True
     if not args.no_cpu_baseline:
         smp = oracle_sample(cfg, G, ops, xi_h, vbar_h, v_gpu_h, target_s=args.cpu_seconds)
@@ -503,6 +540,8 @@ def main():
     ap.add_argument("--dtype", default="", choices=["", "f32", "f64"])
     ap.add_argument("--ops", default="", help="subset of the step to run (default: the ops BASELINE.json lists for "
                                               "the configuration; config 3: forward,inverse,logdet,vjp)")
+    ap.add_argument("--multi", type=int, default=0, help="also time gp_forward_multi / gp_inverse_multi with this many "
+                                                         "samples per call (reported under \"multi\")")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=30.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--reference-points", type=int, default=1 << 16)

@@ -49,7 +49,8 @@ typedef enum {
 
 typedef enum { GP_KERNEL_SE = 0, GP_KERNEL_MATERN32 = 1, GP_KERNEL_EXP = 2 } gp_kernel_kind;
 typedef enum { GP_F32 = 0, GP_F64 = 1 } gp_dtype;
-typedef enum { GP_OP_FORWARD = 0, GP_OP_INVERSE = 1, GP_OP_LOGDET = 2, GP_OP_VJP = 3, GP_OP_BUILD = 4 } gp_op;
+typedef enum { GP_OP_FORWARD = 0, GP_OP_INVERSE = 1, GP_OP_LOGDET = 2, GP_OP_VJP = 3, GP_OP_BUILD = 4,
+               GP_OP_FORWARD_MULTI = 5, GP_OP_INVERSE_MULTI = 6 } gp_op;
 
 /* gp_graph.flags */
 enum {
@@ -115,6 +116,18 @@ gp_status gp_logdet(const gp_graph* g, const gp_kernel* kern, double* logdet_dev
  * Floating-point atomics make the last bits of xi_bar/theta_bar run-dependent.                        */
 gp_status gp_vjp(const gp_graph* g, const gp_kernel* kern, const void* xi, const void* v, const void* v_bar,
                  void* xi_bar, double* theta_bar_dev, void* ws, size_t ws_bytes, void* cuda_stream);
+
+/* Multi-sample apply: S = n_samples noise vectors on one graph and one set of kernel parameters (MGVI /
+ * geoVI "require the forward pass for posterior sampling").  The conditioning of Eq. 2 - K, its
+ * factor, the weights and s - is computed once per point and applied to every sample.  xi, v: device [n][S], row-major
+ * (the S values of a point are contiguous), sample s of these calls equals gp_forward / gp_inverse on column s.
+ * Shapes: fp32 k = 8, 16 and fp64 k = 8 with d = 2, 3 (others: GP_ERR_UNSUPPORTED); 1 <= S <= 1024.
+ * Workspace: gp_workspace_bytes_multi(g, GP_OP_FORWARD_MULTI | GP_OP_INVERSE_MULTI, S).                              */
+size_t gp_workspace_bytes_multi(const gp_graph* g, int32_t op, int32_t n_samples);
+gp_status gp_forward_multi(const gp_graph* g, const gp_kernel* kern, int32_t n_samples, const void* xi, void* v, void* ws,
+                           size_t ws_bytes, void* cuda_stream);
+gp_status gp_inverse_multi(const gp_graph* g, const gp_kernel* kern, int32_t n_samples, const void* v, void* xi, void* ws,
+                           size_t ws_bytes, void* cuda_stream);
 
 /* End-to-end variants with HOST input/output vectors: copy the [n] input host->device into `in_dev`,
  * run the op, copy the [n] result device->host, all on `cuda_stream` (pinned host memory makes the

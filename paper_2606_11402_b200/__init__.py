@@ -18,7 +18,7 @@ from .build import LIB, build_library
 
 GP_OK, GP_ERR_INVALID_ARG, GP_ERR_UNSUPPORTED, GP_ERR_NOT_PD, GP_ERR_CUDA, GP_ERR_WORKSPACE = range(6)
 GP_F32, GP_F64 = 0, 1
-GP_OP_FORWARD, GP_OP_INVERSE, GP_OP_LOGDET, GP_OP_VJP, GP_OP_BUILD = range(5)
+GP_OP_FORWARD, GP_OP_INVERSE, GP_OP_LOGDET, GP_OP_VJP, GP_OP_BUILD, GP_OP_FORWARD_MULTI, GP_OP_INVERSE_MULTI = range(7)
 GP_FLAG_PER_BATCH_LAUNCH, GP_FLAG_GENERIC_KERNEL, GP_FLAG_FLOW_CARRY, GP_FLAG_FLOW_WEIGHTS = 1, 2, 4, 8
 GP_BUILD_SPATIAL_BATCHES, GP_BUILD_RADIUS_CLASSES = 1, 2
 KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
@@ -26,7 +26,7 @@ KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
 EXPORTS = ["gp_workspace_bytes", "gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host",
            "gp_inverse_host", "gp_logdet_host", "gp_vjp_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
            "gp_check_errors", "gp_status_string", "gp_has_specialised", "gp_launch_count", "gp_kernel_time_enable",
-           "gp_kernel_time_last", "gp_measure_alu_peak"]
+           "gp_kernel_time_last", "gp_measure_alu_peak", "gp_workspace_bytes_multi", "gp_forward_multi", "gp_inverse_multi"]
 
 
 class GraphGPError(RuntimeError):
@@ -83,6 +83,12 @@ def lib():
                                      vp, vp, vp, C.c_int32, C.POINTER(C.c_int32), vp, sz, vp]
         L.gp_graph_build_times.argtypes = [vp, vp]
         L.gp_check_errors.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.gp_workspace_bytes_multi.restype = C.c_size_t
+        L.gp_workspace_bytes_multi.argtypes = [C.POINTER(_Graph), C.c_int32, C.c_int32]
+        L.gp_forward_multi.argtypes = gk + [C.c_int32, vp, vp, vp, sz, vp]
+        L.gp_inverse_multi.argtypes = gk + [C.c_int32, vp, vp, vp, sz, vp]
+        L.gp_forward_multi.restype = C.c_int
+        L.gp_inverse_multi.restype = C.c_int
         L.gp_measure_alu_peak.argtypes = [vp, C.c_int32, vp, sz, vp]
         L.gp_measure_alu_peak.restype = C.c_int
         for name in ("gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host", "gp_inverse_host",
@@ -311,6 +317,38 @@ def gp_vjp(graph: Graph, kern: Kernel, xi, v, v_bar, stream=None):
     _check(lib().gp_vjp(C.byref(g), C.byref(k), xi.data_ptr(), v.data_ptr(), v_bar.data_ptr(), xi_bar.data_ptr(),
                         tb.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "gp_vjp")
     return xi_bar, tb
+
+
+def _multi(graph: Graph, kern: Kernel, op: int, name: str, src, out, stream):
+    torch = _torch()
+    want = torch.float64 if graph.dtype_id == GP_F64 else torch.float32
+    if src.dim() != 2 or src.shape[0] != graph.n or src.dtype != want or not src.is_contiguous() or src.device != graph.x.device:
+        raise ValueError(f"{name}: expected a contiguous [n, S] tensor of the graph's dtype on the graph's device")
+    S = int(src.shape[1])
+    if out is None:
+        out = torch.empty_like(src)
+    elif out.shape != src.shape or out.dtype != src.dtype or not out.is_contiguous() or out.device != src.device:
+        raise ValueError(f"{name}: out must match the input")
+    g, k = graph.c(), kern.c()
+    need = int(lib().gp_workspace_bytes_multi(C.byref(g), op, S))
+    key = (op, S)
+    ws = graph._ws.get(key)
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(max(need, 256), dtype=torch.uint8, device=graph.x.device)
+        graph._ws[key] = ws
+    fn = lib().gp_forward_multi if op == GP_OP_FORWARD_MULTI else lib().gp_inverse_multi
+    _check(fn(C.byref(g), C.byref(k), S, src.data_ptr(), out.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)), name)
+    return out
+
+
+def gp_forward_multi(graph: Graph, kern: Kernel, xi, out=None, stream=None):
+    """S samples at once: xi, v device [n, S]; column s equals gp_forward on xi[:, s]."""
+    return _multi(graph, kern, GP_OP_FORWARD_MULTI, "gp_forward_multi", xi, out, stream)
+
+
+def gp_inverse_multi(graph: Graph, kern: Kernel, v, out=None, stream=None):
+    """S samples at once: v, xi device [n, S]; column s equals gp_inverse on v[:, s]."""
+    return _multi(graph, kern, GP_OP_INVERSE_MULTI, "gp_inverse_multi", v, out, stream)
 
 
 def gp_forward_host(graph: Graph, kern: Kernel, xi_host, v_host, in_dev, out_dev, stream=None):

@@ -85,7 +85,7 @@ gp_status ktime_end(cudaStream_t st) {
   return GP_OK;
 }
 
-static gp_status validate(const gp_graph* g, const gp_kernel* kern) {
+gp_status validate_graph(const gp_graph* g, const gp_kernel* kern) {
   if (!g || !kern) return GP_ERR_INVALID_ARG;
   if (g->n <= 0 || g->n0 < 0 || g->n0 > g->n) return GP_ERR_INVALID_ARG;
   if (g->dtype != GP_F32 && g->dtype != GP_F64) return GP_ERR_INVALID_ARG;
@@ -110,7 +110,7 @@ static gp_status validate(const gp_graph* g, const gp_kernel* kern) {
 
 static gp_status make_ctx(const gp_graph* g, const gp_kernel* kern, int op, void* ws, size_t ws_bytes,
                           void* stream, OpCtx* out) {
-  GP_OK_OR_RETURN(validate(g, kern));
+  GP_OK_OR_RETURN(validate_graph(g, kern));
   WsLayout lay = ws_layout(g, op);
   if (!ws || ws_bytes < lay.total || (((uintptr_t)ws) & 255) != 0) return GP_ERR_WORKSPACE;
   int ndev = 0;

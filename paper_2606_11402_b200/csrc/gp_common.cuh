@@ -248,7 +248,10 @@ gp_status ktime_end(cudaStream_t st);
 // overlapped: the factorisation runs beside the bulk kernel on the side stream -> use few CTAs so that most
 // SMs keep their full bulk occupancy; otherwise (forward: the head is on the critical path) one CTA per SM.
 gp_status head_factor(const OpCtx& c, const void* carried_src /*dtype [n0] or null*/, int n_carried, bool overlapped = false);
+// build + factor with `n_carried` extra rows that the caller has already written below the square part
+gp_status head_factor_preinit(const OpCtx& c, int n_carried, bool overlapped);
 gp_status head_forward(const OpCtx& c, const void* xi, void* v, void* rec, bool rec_is_packed);
+gp_status validate_graph(const gp_graph* g, const gp_kernel* kern);   // gp_api.cu: synchronous argument checks
 gp_status head_inverse_out(const OpCtx& c, void* xi);
 gp_status head_logdet(const OpCtx& c, double* acc /*device: acc[0] += logdet head*/,
                       double* grad_ell_acc /*device or null: += ell * d/dell, needs head_factor(c, nullptr, 2 n0)*/);

@@ -234,17 +234,50 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
   }
 }
 
+static gp_status head_build(const OpCtx& c) {
+  const int n0 = (int)c.g->n0;
+  KParams<double> kp = make_kparams<double>(*c.kern);
+  dim3 bb(16, 16), bg((n0 + 15) / 16, (n0 + 15) / 16);
+  if (c.g->dtype == GP_F64)
+    head_build_kernel<double><<<bg, bb, 0, c.st>>>((const double*)c.g->x, c.g->d, n0, c.kern->kind, kp, c.head());
+  else
+    head_build_kernel<float><<<bg, bb, 0, c.st>>>((const float*)c.g->x, c.g->d, n0, c.kern->kind, kp, c.head());
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+static gp_status head_chol(const OpCtx& c, int n_carried, bool overlapped) {
+  const int n0 = (int)c.g->n0;
+  double* A = c.head();
+  int rows_total = n0 + n_carried;
+  const int grid_ctas = device_sm_count();                  // one CTA per SM: all co-resident
+  if (grid_ctas <= 0) return GP_ERR_CUDA;
+  int n0_arg = n0;
+  Control* ctrl = c.ctrl();
+  void* args[] = {(void*)&A, (void*)&n0_arg, (void*)&rows_total, (void*)&ctrl};
+  int ctas = grid_ctas;
+  if (overlapped) {                                         // a quarter of the SMs; more when many rows are carried
+    ctas = n_carried > n0 ? grid_ctas / 2 : grid_ctas / 4;
+    if (ctas < 1) ctas = 1;
+  }
+  GP_CUDA_OK(cudaLaunchCooperativeKernel((const void*)head_chol_kernel, dim3(ctas), dim3(256), args, 0, c.st));
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+gp_status head_factor_preinit(const OpCtx& c, int n_carried, bool overlapped) {
+  if (c.g->n0 <= 0) return GP_OK;
+  GP_OK_OR_RETURN(head_build(c));
+  return head_chol(c, n_carried, overlapped);
+}
+
 gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried, bool overlapped) {
   const int n0 = (int)c.g->n0;
   if (n0 <= 0) return GP_OK;
   double* A = c.head();
   KParams<double> kp = make_kparams<double>(*c.kern);
   dim3 bb(16, 16), bg((n0 + 15) / 16, (n0 + 15) / 16);
-  if (c.g->dtype == GP_F64)
-    head_build_kernel<double><<<bg, bb, 0, c.st>>>((const double*)c.g->x, c.g->d, n0, c.kern->kind, kp, A);
-  else
-    head_build_kernel<float><<<bg, bb, 0, c.st>>>((const float*)c.g->x, c.g->d, n0, c.kern->kind, kp, A);
-  GP_LAUNCH_CHECK();
+  GP_OK_OR_RETURN(head_build(c));
   if (n_carried == 2 * n0 && n_carried > 1) {
     if (c.g->dtype == GP_F64)
       head_carry_grad_init_kernel<double><<<bg, bb, 0, c.st>>>((const double*)c.g->x, c.g->d, n0, c.kern->kind, kp, A);
@@ -261,20 +294,7 @@ gp_status head_factor(const OpCtx& c, const void* carried_src, int n_carried, bo
       head_carry_init_kernel<float><<<grid, 256, 0, c.st>>>((const float*)carried_src, n0, mode, A);
     GP_LAUNCH_CHECK();
   }
-  int rows_total = n0 + n_carried;
-  const int grid_ctas = device_sm_count();                  // one CTA per SM: all co-resident
-  if (grid_ctas <= 0) return GP_ERR_CUDA;
-  int n0_arg = n0;
-  Control* ctrl = c.ctrl();
-  void* args[] = {(void*)&A, (void*)&n0_arg, (void*)&rows_total, (void*)&ctrl};
-  int ctas = grid_ctas;
-  if (overlapped) {                                         // a quarter of the SMs; more when many rows are carried
-    ctas = n_carried > n0 ? grid_ctas / 2 : grid_ctas / 4;
-    if (ctas < 1) ctas = 1;
-  }
-  GP_CUDA_OK(cudaLaunchCooperativeKernel((const void*)head_chol_kernel, dim3(ctas), dim3(256), args, 0, c.st));
-  GP_LAUNCH_CHECK();
-  return GP_OK;
+  return head_chol(c, n_carried, overlapped);
 }
 
 // v_head = sigma * L xi_head  (one warp per row)
