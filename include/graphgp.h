@@ -129,9 +129,12 @@ gp_status gp_forward_multi(const gp_graph* g, const gp_kernel* kern, int32_t n_s
 gp_status gp_inverse_multi(const gp_graph* g, const gp_kernel* kern, int32_t n_samples, const void* v, void* xi, void* ws,
                            size_t ws_bytes, void* cuda_stream);
 
-/* End-to-end variants with HOST input/output vectors: copy the [n] input host->device into `in_dev`,
- * run the op, copy the [n] result device->host, all on `cuda_stream` (pinned host memory makes the
- * copies asynchronous).  The graph stays device-resident.  in_dev/out_dev: device staging, [n] each.  */
+/* End-to-end variants with HOST input/output vectors: the [n] input goes host->device into `in_dev`, the op runs,
+ * the [n] result goes device->host (pinned host memory makes the copies asynchronous).  The graph stays device-
+ * resident.  in_dev/out_dev: device staging, [n] each.  The op is cut into ranges of the graph order (a point reads
+ * only points before it) and the copies of neighbouring ranges run on two library-internal copy streams (per device,
+ * created on first use) beside the kernels; everything is ordered after the work already queued on `cuda_stream`,
+ * and `cuda_stream` ends only when the result is on the host: the caller synchronises that stream and reads.        */
 gp_status gp_forward_host(const gp_graph* g, const gp_kernel* kern, const void* xi_host, void* v_host,
                           void* in_dev, void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream);
 gp_status gp_inverse_host(const gp_graph* g, const gp_kernel* kern, const void* v_host, void* xi_host,

@@ -46,6 +46,20 @@ gp_status side_stream(SideStream** out) {
   *out = &s;
   return GP_OK;
 }
+gp_status copy_streams(cudaStream_t* cin, cudaStream_t* cout) {
+  static cudaStream_t per_dev[64][2];
+  int dev = 0;
+  GP_CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return GP_ERR_CUDA;
+  std::lock_guard<std::mutex> lock(g_dev_mutex[dev]);
+  if (!per_dev[dev][0]) {
+    GP_CUDA_OK(cudaStreamCreateWithFlags(&per_dev[dev][0], cudaStreamNonBlocking));
+    GP_CUDA_OK(cudaStreamCreateWithFlags(&per_dev[dev][1], cudaStreamNonBlocking));
+  }
+  *cin = per_dev[dev][0];
+  *cout = per_dev[dev][1];
+  return GP_OK;
+}
 gp_status side_fork(const SideStream* s, cudaStream_t main) {
   std::lock_guard<std::mutex> lock(g_dev_mutex[s->device]);
   GP_CUDA_OK(cudaEventRecord(s->fork, main));
@@ -165,23 +179,27 @@ gp_status gp_vjp(const gp_graph* g, const gp_kernel* kern, const void* xi, const
 gp_status gp_forward_host(const gp_graph* g, const gp_kernel* kern, const void* xi_host, void* v_host, void* in_dev,
                           void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream) {
   if (!g || !xi_host || !v_host || !in_dev || !out_dev) return GP_ERR_INVALID_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  size_t bytes = (size_t)g->n * dtype_bytes(g->dtype);
-  GP_CUDA_OK(cudaMemcpyAsync(in_dev, xi_host, bytes, cudaMemcpyHostToDevice, st));
-  GP_OK_OR_RETURN(gp_forward(g, kern, in_dev, out_dev, ws, ws_bytes, cuda_stream));
-  GP_CUDA_OK(cudaMemcpyAsync(v_host, out_dev, bytes, cudaMemcpyDeviceToHost, st));
-  return GP_OK;
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_FORWARD, ws, ws_bytes, cuda_stream, &c));
+  HostIO io;
+  io.in_host[0] = xi_host;
+  io.out_host = v_host;
+  GP_OK_OR_RETURN(copy_streams(&io.cin, &io.cout));
+  c.io = &io;
+  return run_forward(c, in_dev, out_dev);
 }
 
 gp_status gp_inverse_host(const gp_graph* g, const gp_kernel* kern, const void* v_host, void* xi_host, void* in_dev,
                           void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream) {
   if (!g || !xi_host || !v_host || !in_dev || !out_dev) return GP_ERR_INVALID_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  size_t bytes = (size_t)g->n * dtype_bytes(g->dtype);
-  GP_CUDA_OK(cudaMemcpyAsync(in_dev, v_host, bytes, cudaMemcpyHostToDevice, st));
-  GP_OK_OR_RETURN(gp_inverse(g, kern, in_dev, out_dev, ws, ws_bytes, cuda_stream));
-  GP_CUDA_OK(cudaMemcpyAsync(xi_host, out_dev, bytes, cudaMemcpyDeviceToHost, st));
-  return GP_OK;
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_INVERSE, ws, ws_bytes, cuda_stream, &c));
+  HostIO io;
+  io.in_host[0] = v_host;
+  io.out_host = xi_host;
+  GP_OK_OR_RETURN(copy_streams(&io.cin, &io.cout));
+  c.io = &io;
+  return run_inverse(c, in_dev, out_dev);
 }
 
 gp_status gp_logdet_host(const gp_graph* g, const gp_kernel* kern, double* logdet_host, double* dlogdet_dtheta_host,
@@ -202,14 +220,17 @@ gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_h
   if (!g || !xi_host || !v_host || !v_bar_host || !xi_bar_host || !theta_bar_host || !xi_dev || !v_dev || !v_bar_dev ||
       !xi_bar_dev || !theta_bar_dev)
     return GP_ERR_INVALID_ARG;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  size_t bytes = (size_t)g->n * dtype_bytes(g->dtype);
-  GP_CUDA_OK(cudaMemcpyAsync(xi_dev, xi_host, bytes, cudaMemcpyHostToDevice, st));
-  GP_CUDA_OK(cudaMemcpyAsync(v_dev, v_host, bytes, cudaMemcpyHostToDevice, st));
-  GP_CUDA_OK(cudaMemcpyAsync(v_bar_dev, v_bar_host, bytes, cudaMemcpyHostToDevice, st));
-  GP_OK_OR_RETURN(gp_vjp(g, kern, xi_dev, v_dev, v_bar_dev, xi_bar_dev, theta_bar_dev, ws, ws_bytes, cuda_stream));
-  GP_CUDA_OK(cudaMemcpyAsync(xi_bar_host, xi_bar_dev, bytes, cudaMemcpyDeviceToHost, st));
-  GP_CUDA_OK(cudaMemcpyAsync(theta_bar_host, theta_bar_dev, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_VJP, ws, ws_bytes, cuda_stream, &c));
+  HostIO io;
+  io.in_host[0] = xi_host;
+  io.in_host[1] = v_host;
+  io.in_host[2] = v_bar_host;
+  io.out_host = xi_bar_host;
+  GP_OK_OR_RETURN(copy_streams(&io.cin, &io.cout));
+  c.io = &io;
+  GP_OK_OR_RETURN(run_vjp(c, xi_dev, v_dev, v_bar_dev, xi_bar_dev, theta_bar_dev));
+  GP_CUDA_OK(cudaMemcpyAsync(theta_bar_host, theta_bar_dev, 2 * sizeof(double), cudaMemcpyDeviceToHost, (cudaStream_t)cuda_stream));
   return GP_OK;
 }
 

@@ -209,12 +209,43 @@ inline WsLayout ws_layout(const gp_graph* g, int op) {
   return w;
 }
 
+// Host-buffer variants (gp_*_host): the [n] inputs live in (pinned) host memory and the result goes back to it.  The
+// op is cut into ranges of the graph order (a point only reads points before it) so that the host->device copy of a
+// later range and the device->host copy of an earlier one run on two library-internal copy streams beside the kernels.
+struct HostIO {
+  const void* in_host[3] = {nullptr, nullptr, nullptr};   // forward: xi; inverse: v; vjp: xi, v, v_bar
+  void* out_host = nullptr;
+  cudaStream_t cin = nullptr, cout = nullptr;
+};
+gp_status copy_streams(cudaStream_t* cin, cudaStream_t* cout);   // per device, created on first use, never destroyed
+
+// events of one call (no timing); destroyed when the call returns (CUDA releases them once they have completed)
+struct EventBag {
+  cudaEvent_t ev[64];
+  int used = 0;
+  cudaEvent_t make() {
+    if (used >= 64) return nullptr;
+    if (cudaEventCreateWithFlags(&ev[used], cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    return ev[used++];
+  }
+  ~EventBag() { for (int i = 0; i < used; ++i) cudaEventDestroy(ev[i]); }
+};
+// `waiter` waits for everything queued on `src` so far
+inline gp_status stream_after(EventBag& bag, cudaStream_t waiter, cudaStream_t src) {
+  cudaEvent_t e = bag.make();
+  if (!e) return GP_ERR_CUDA;
+  if (cudaEventRecord(e, src) != cudaSuccess) return GP_ERR_CUDA;
+  if (cudaStreamWaitEvent(waiter, e, 0) != cudaSuccess) return GP_ERR_CUDA;
+  return GP_OK;
+}
+
 struct OpCtx {
   const gp_graph* g;
   const gp_kernel* kern;
   char* ws;
   WsLayout lay;
   cudaStream_t st;
+  const HostIO* io = nullptr;
   Control* ctrl() const { return (Control*)(ws + lay.ctrl_off); }
   int64_t* boff_dev() const { return (int64_t*)(ws + lay.boff_off); }
   void* gtab() const { return ws + lay.gtab_off; }

@@ -503,13 +503,19 @@ static gp_status launch_range(const OpCtx& c, bool spec, const T* vals, const T*
 }
 
 template <typename T>
-static gp_status pack(const OpCtx& c, const T* vals, bool pending = false) {
-  int64_t n = c.g->n;
-  unsigned grid = (unsigned)((n + 255) / 256);
-  pack_kernel<T><<<grid, 256, 0, c.st>>>((const T*)c.g->x, vals, (Rec<T>*)c.rec(), n, c.g->d, pending ? 1 : 0);
+static gp_status pack(const OpCtx& c, const T* vals, bool pending = false, int64_t lo = 0, int64_t hi = -1) {
+  if (hi < 0) hi = c.g->n;
+  const int64_t cnt = hi - lo;
+  if (cnt <= 0) return GP_OK;
+  unsigned grid = (unsigned)((cnt + 255) / 256);
+  pack_kernel<T><<<grid, 256, 0, c.st>>>((const T*)c.g->x + lo * c.g->d, vals ? vals + lo : nullptr, (Rec<T>*)c.rec() + lo, cnt,
+                                         c.g->d, pending ? 1 : 0);
   GP_LAUNCH_CHECK();
   return GP_OK;
 }
+
+// ranges of the graph order for the host-buffer variants: about kHostChunks pieces, the first starting at 0
+constexpr int kHostChunks = 4;
 
 // grad = d/d(sigma, ell):  every point contributes log sigma^2 + log s_i^2, so d/dsigma = 2 N / sigma exactly;
 // acc[2] holds ell * d/dell (gp_vjp.cu).
@@ -519,6 +525,26 @@ __global__ void finalize_logdet_kernel(const Control* ctrl, double* logdet, doub
     logdet[0] = ctrl->acc[0];
     if (grad) { grad[0] = two_n_over_sigma; grad[1] = ctrl->acc[2] * inv_ell; }
   }
+}
+
+// host-buffer forward: xi[0 : cut) has arrived when the first kernel starts, the rest when `arrived_rest` fires; v leaves
+// stretch by stretch on the copy-out stream
+struct ForwardPipe {
+  int64_t cut;
+  cudaEvent_t arrived_rest;
+  EventBag* bag;
+  bool waited;
+};
+static int64_t forward_pipe_cut(const OpCtx& c) {
+  // first batch boundary past an eighth of the conditioned points, or the first batch larger than twice what the GPU
+  // holds in flight (where launch_flow starts its large-batch stretch), whichever comes first
+  const int L = c.g->n_batches;
+  const int64_t* off = c.g->batch_off;
+  const int64_t n = c.g->n, n0 = c.g->n0;
+  const int64_t large = 2 * (int64_t)device_sm_count() * GP_FLOW_MIN_CTAS * kCondThreads;
+  for (int b = 0; b < L; ++b)
+    if (off[b + 1] - off[b] >= large || off[b] - n0 >= (n - n0) / 8) return off[b];
+  return n;
 }
 
 template <typename T, int K, int D, int MODE>
@@ -550,7 +576,7 @@ static gp_status launch_flow_segment(const OpCtx& c, const T* xi, T* v, int64_t 
 // own ticket counter.  The per-batch table {first group, first point} goes to the workspace (pageable source: staged
 // by the runtime before the copy call returns); flow_groups_kernel expands it to one entry per 128-point group.
 template <typename T, int K, int D>
-static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
+static gp_status launch_flow(const OpCtx& c, const T* xi, T* v, ForwardPipe* fp) {
   const int L = c.g->n_batches;
   if (L <= 0) return GP_OK;
   const int64_t* off = c.g->batch_off;
@@ -582,10 +608,19 @@ static gp_status launch_flow(const OpCtx& c, const T* xi, T* v) {
     int e = b + 1;
     // the last ticket counter takes everything that is left (the wait-last body is right for any batch size)
     if (slot == kFlowTickets - 1) e = L;
-    else while (e < L && is_big(e) == big) ++e;
+    else while (e < L && is_big(e) == big && !(fp && big && off[e] - off[b] >= (c.g->n - c.g->n0) / 5)) ++e;
+    if (fp && !fp->waited && off[e] > fp->cut) {              // this stretch reads xi beyond what has arrived
+      GP_CUDA_OK(cudaStreamWaitEvent(c.st, fp->arrived_rest, 0));
+      fp->waited = true;
+    }
     const int64_t g0 = tab[2 * b], ng = tab[2 * e] - tab[2 * b];
     if (big && slot != kFlowTickets - 1) GP_OK_OR_RETURN((launch_flow_segment<T, K, D, FLOW_CARRY>(c, xi, v, g0, ng, slot)));
     else GP_OK_OR_RETURN((launch_flow_segment<T, K, D, FLOW_WEIGHTS>(c, xi, v, g0, ng, slot)));
+    if (fp) {                                                 // v of this stretch (and of the head) goes home
+      const int64_t lo = b == 0 ? 0 : off[b], hi = off[e];
+      GP_OK_OR_RETURN(stream_after(*fp->bag, c.io->cout, c.st));
+      GP_CUDA_OK(cudaMemcpyAsync((T*)c.io->out_host + lo, v + lo, (size_t)(hi - lo) * sizeof(T), cudaMemcpyDeviceToHost, c.io->cout));
+    }
     b = e;
     ++slot;
   }
@@ -653,6 +688,22 @@ static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
 #undef X
   }
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
+  EventBag bag;
+  ForwardPipe pipe{c.g->n, nullptr, &bag, false};
+  if (c.io) {   // host-buffer variant: xi arrives in two parts on the copy-in stream
+    const int64_t n = c.g->n;
+    pipe.cut = forward_pipe_cut(c);
+    GP_OK_OR_RETURN(stream_after(bag, c.io->cin, c.st));
+    GP_CUDA_OK(cudaMemcpyAsync((T*)xi, c.io->in_host[0], (size_t)pipe.cut * sizeof(T), cudaMemcpyHostToDevice, c.io->cin));
+    GP_OK_OR_RETURN(stream_after(bag, c.st, c.io->cin));
+    if (pipe.cut < n)
+      GP_CUDA_OK(cudaMemcpyAsync((T*)xi + pipe.cut, (const T*)c.io->in_host[0] + pipe.cut, (size_t)(n - pipe.cut) * sizeof(T),
+                                 cudaMemcpyHostToDevice, c.io->cin));
+    pipe.arrived_rest = bag.make();
+    if (!pipe.arrived_rest) return GP_ERR_CUDA;
+    GP_CUDA_OK(cudaEventRecord(pipe.arrived_rest, c.io->cin));
+  }
+  ForwardPipe* fp = c.io ? &pipe : nullptr;
   // the head is on the critical path (every batch depends on it); packing the records is not: side stream
   SideStream* side = nullptr;
   GP_OK_OR_RETURN(side_stream(&side));
@@ -669,40 +720,82 @@ static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
   if (flow) {
 #define X(TT, K, D) \
     if constexpr (std::is_same<TT, T>::value) {                    \
-      if (c.g->k == K && c.g->d == D) { GP_OK_OR_RETURN((launch_flow<T, K, D>(c, xi, v))); return ktime_end(c.st); } \
+      if (c.g->k == K && c.g->d == D) {                            \
+        GP_OK_OR_RETURN((launch_flow<T, K, D>(c, xi, v, fp)));     \
+        GP_OK_OR_RETURN(ktime_end(c.st));                          \
+        if (fp) GP_OK_OR_RETURN(stream_after(bag, c.st, c.io->cout)); \
+        return GP_OK;                                              \
+      }                                                            \
     }
     GP_SPEC_TABLE(X)
 #undef X
 #define X(TT, K, D, L) \
     if constexpr (std::is_same<TT, T>::value) {                    \
-      if (c.g->k == K && c.g->d == D) { GP_OK_OR_RETURN((launch_lg_flow<T, K, D, L>(c, xi, v))); return ktime_end(c.st); } \
+      if (c.g->k == K && c.g->d == D) {                            \
+        if (fp) GP_CUDA_OK(cudaStreamWaitEvent(c.st, fp->arrived_rest, 0)); \
+        GP_OK_OR_RETURN((launch_lg_flow<T, K, D, L>(c, xi, v)));   \
+        GP_OK_OR_RETURN(ktime_end(c.st));                          \
+        if (fp) GP_CUDA_OK(cudaMemcpyAsync(c.io->out_host, v, (size_t)c.g->n * sizeof(T), cudaMemcpyDeviceToHost, c.st)); \
+        return GP_OK;                                              \
+      }                                                            \
     }
     GP_LG_TABLE(X)
 #undef X
   }
   const int64_t* off = c.g->batch_off;
+  if (fp) GP_CUDA_OK(cudaStreamWaitEvent(c.st, fp->arrived_rest, 0));
   for (int b = 0; b < c.g->n_batches; ++b)
     GP_OK_OR_RETURN((launch_range<T, OPK_FORWARD>(c, spec, v, xi, v, off[b], off[b + 1])));
-  return ktime_end(c.st);
+  GP_OK_OR_RETURN(ktime_end(c.st));
+  if (fp) GP_CUDA_OK(cudaMemcpyAsync(c.io->out_host, v, (size_t)c.g->n * sizeof(T), cudaMemcpyDeviceToHost, c.st));
+  return GP_OK;
 }
 
 template <typename T>
 static gp_status inverse_t(const OpCtx& c, const T* v, T* xi) {
   bool spec = use_spec(c);
+  const int64_t n = c.g->n, n0 = c.g->n0;
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
+  EventBag bag;
+  // host-buffer variant: v arrives range by range (a point reads only points before it), xi leaves range by range
+  const int chunks = c.io ? kHostChunks : 1;
+  int64_t cut[kHostChunks + 1];
+  for (int q = 0; q <= chunks; ++q) cut[q] = q == 0 ? 0 : (q == chunks ? n : n0 + (n - n0) * q / chunks);
+  cudaEvent_t arrived[kHostChunks] = {};
+  if (c.io) {
+    GP_OK_OR_RETURN(stream_after(bag, c.io->cin, c.st));       // the staging buffer may still be read by earlier work
+    for (int q = 0; q < chunks; ++q) {
+      GP_CUDA_OK(cudaMemcpyAsync((T*)v + cut[q], (const T*)c.io->in_host[0] + cut[q], (size_t)(cut[q + 1] - cut[q]) * sizeof(T),
+                                 cudaMemcpyHostToDevice, c.io->cin));
+      arrived[q] = bag.make();
+      if (!arrived[q]) return GP_ERR_CUDA;
+      GP_CUDA_OK(cudaEventRecord(arrived[q], c.io->cin));
+    }
+  }
   // the head (xi[0:n0]) and the bulk (xi[n0:n]) are independent: head on the side stream, submitted first
   SideStream* side = nullptr;
   GP_OK_OR_RETURN(side_stream(&side));
+  if (c.io) GP_CUDA_OK(cudaStreamWaitEvent(c.st, arrived[0], 0));
   GP_OK_OR_RETURN(side_fork(side, c.st));
   OpCtx hc = c;
   hc.st = side->stream;
   GP_OK_OR_RETURN(head_factor(hc, v, 1, true));
   GP_OK_OR_RETURN(head_inverse_out(hc, xi));
-  if (spec) GP_OK_OR_RETURN(pack<T>(c, v));
   GP_OK_OR_RETURN(ktime_begin(c.st));
-  GP_OK_OR_RETURN((launch_range<T, OPK_INVERSE>(c, spec, v, v, xi, c.g->n0, c.g->n)));
+  for (int q = 0; q < chunks; ++q) {
+    if (c.io && q > 0) GP_CUDA_OK(cudaStreamWaitEvent(c.st, arrived[q], 0));
+    if (spec) GP_OK_OR_RETURN(pack<T>(c, v, false, cut[q], cut[q + 1]));
+    GP_OK_OR_RETURN((launch_range<T, OPK_INVERSE>(c, spec, v, v, xi, cut[q] < n0 ? n0 : cut[q], cut[q + 1])));
+    if (q == 0) GP_OK_OR_RETURN(side_join(side, c.st));
+    if (c.io) {
+      GP_OK_OR_RETURN(stream_after(bag, c.io->cout, c.st));
+      GP_CUDA_OK(cudaMemcpyAsync((T*)c.io->out_host + cut[q], xi + cut[q], (size_t)(cut[q + 1] - cut[q]) * sizeof(T),
+                                 cudaMemcpyDeviceToHost, c.io->cout));
+    }
+  }
   GP_OK_OR_RETURN(ktime_end(c.st));
-  return side_join(side, c.st);
+  if (c.io) GP_OK_OR_RETURN(stream_after(bag, c.st, c.io->cout));   // the caller's stream ends when the result is on the host
+  return GP_OK;
 }
 
 template <typename T>

@@ -196,10 +196,10 @@ logdet_grad_pk_kernel(const Rec<float>* __restrict__ rec, const int32_t* __restr
 template <int K, int D, int KIND>
 __global__ void __launch_bounds__(kGradThreads, GP_GRAD_MIN_CTAS)
 vjp_geom_kernel(const Rec<float>* __restrict__ rec, const int32_t* __restrict__ nbr, const float* __restrict__ xi,
-                float* __restrict__ wbuf, float4* __restrict__ sab, int64_t n0, int64_t n, KParams<float> kp,
+                float* __restrict__ wbuf, float4* __restrict__ sab, int64_t n0, int64_t first, int64_t n, KParams<float> kp,
                 Control* ctrl) {
   extern __shared__ float4 dq_raw[];
-  const int64_t i = n0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t i = first + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // points [first, n) of this launch
   if (i >= n) return;
   DqStore<K> dq = dq_store_of<K>(dq_raw);
   Rec<float> self = load_rec<false>(rec + i);
@@ -480,8 +480,33 @@ static gp_status launch_logdet_grad_pk(const OpCtx& c) {
   return GP_OK;
 }
 
+// geometry of the points [first, end): everything of the VJP that does not depend on the incoming cotangent
 template <int K, int D>
-static gp_status launch_vjp_flow(const OpCtx& c, const float* xi, float* gbar, float* xibar) {
+static gp_status launch_vjp_geom(const OpCtx& c, const float* xi, int64_t first, int64_t end) {
+  const int64_t cnt = end - first, total = c.g->n - c.g->n0;
+  if (cnt <= 0) return GP_OK;
+  KParams<float> kp = make_kparams<float>(*c.kern);
+  const Rec<float>* rec = (const Rec<float>*)c.rec();
+  float* wbuf = c.wbuf();
+  float4* sab = reinterpret_cast<float4*>(wbuf + (size_t)total * K);
+  size_t smem = dq_smem_bytes(K, kGradThreads);
+  unsigned ggrid = (unsigned)((cnt + kGradThreads - 1) / kGradThreads);
+#define GP_VF(KIND)                                                                                              \
+  GP_OK_OR_RETURN(set_dq_smem(vjp_geom_kernel<K, D, KIND>, smem));                                              \
+  vjp_geom_kernel<K, D, KIND><<<ggrid, kGradThreads, smem, c.st>>>(rec, c.g->nbr, xi, wbuf, sab, c.g->n0, first, end, kp, c.ctrl());
+  switch (c.kern->kind) {
+    case GP_KERNEL_SE: GP_VF(GP_KERNEL_SE) break;
+    case GP_KERNEL_MATERN32: GP_VF(GP_KERNEL_MATERN32) break;
+    default: GP_VF(GP_KERNEL_EXP) break;
+  }
+#undef GP_VF
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+
+// the reverse sweep proper over all batches (ticketed dataflow, last batch first)
+template <int K>
+static gp_status launch_vjp_scatter(const OpCtx& c, float* gbar, float* xibar) {
   const int L = c.g->n_batches;
   const int64_t cnt = c.g->n - c.g->n0;
   if (L <= 0 || cnt <= 0) return GP_OK;
@@ -501,25 +526,11 @@ static gp_status launch_vjp_flow(const OpCtx& c, const float* xi, float* gbar, f
   if (chunks <= 0 || chunks > 0x7fffffffLL) return GP_ERR_UNSUPPORTED;
   // pageable source: the runtime stages it before returning, so the vector may die afterwards
   GP_CUDA_OK(cudaMemcpyAsync(c.boff_dev(), tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, c.st));
-  KParams<float> kp = make_kparams<float>(*c.kern);
-  const Rec<float>* rec = (const Rec<float>*)c.rec();
   const longlong4* tab_d = (const longlong4*)c.boff_dev();
   float* wbuf = c.wbuf();
   float4* sab = reinterpret_cast<float4*>(wbuf + (size_t)cnt * K);
-  size_t smem = dq_smem_bytes(K, kGradThreads);
-  unsigned ggrid = (unsigned)((cnt + kGradThreads - 1) / kGradThreads);
-#define GP_VF(KIND)                                                                                              \
-  GP_OK_OR_RETURN(set_dq_smem(vjp_geom_kernel<K, D, KIND>, smem));                                              \
-  vjp_geom_kernel<K, D, KIND><<<ggrid, kGradThreads, smem, c.st>>>(rec, c.g->nbr, xi, wbuf, sab, c.g->n0, c.g->n, kp, c.ctrl());
-  switch (c.kern->kind) {
-    case GP_KERNEL_SE: GP_VF(GP_KERNEL_SE) break;
-    case GP_KERNEL_MATERN32: GP_VF(GP_KERNEL_MATERN32) break;
-    default: GP_VF(GP_KERNEL_EXP) break;
-  }
-#undef GP_VF
-  GP_LAUNCH_CHECK();
   vjp_scatter_kernel<K><<<(unsigned)chunks, kScatterThreads, 0, c.st>>>(c.g->nbr, wbuf, sab, gbar, xibar, tab_d, L, c.g->n0,
-                                                                      c.g->n, kp.sigma, c.ctrl());
+                                                                      c.g->n, (float)c.kern->sigma, c.ctrl());
   GP_LAUNCH_CHECK();
   return GP_OK;
 }
@@ -532,8 +543,38 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
   bool spec = grad_use_spec(c);
   const int64_t n = c.g->n, n0 = c.g->n0;
   T* gbar = (T*)c.gbar();
+  bool flow = false;                          // two-phase packed fp32 path
+  if constexpr (std::is_same<T, float>::value) {
+    if (spec && !(c.g->flags & GP_FLAG_PER_BATCH_LAUNCH)) {
+#define X(K, D) \
+      if (c.g->k == K && c.g->d == D) flow = true;
+      GP_GRAD_PK_TABLE(X)
+#undef X
+    }
+  }
   GP_CUDA_OK(cudaMemsetAsync(c.ctrl(), 0, kCtrlBytes, c.st));
-  GP_CUDA_OK(cudaMemcpyAsync(gbar, vbar, (size_t)n * sizeof(T), cudaMemcpyDeviceToDevice, c.st));
+  // host-buffer variant: v and xi arrive range by range beside the geometry kernel (a point reads only points before
+  // it), then v_bar; xi_bar goes home at the end
+  EventBag bag;
+  const int chunks = (c.io && flow) ? 4 : 1;
+  int64_t cut[5];
+  for (int q = 0; q <= chunks; ++q) cut[q] = q == 0 ? 0 : (q == chunks ? n : n0 + (n - n0) * q / chunks);
+  cudaEvent_t arrived[4] = {}, vbar_arrived = nullptr;
+  if (c.io) {
+    GP_OK_OR_RETURN(stream_after(bag, c.io->cin, c.st));
+    for (int q = 0; q < chunks; ++q) {
+      const size_t bytes = (size_t)(cut[q + 1] - cut[q]) * sizeof(T);
+      GP_CUDA_OK(cudaMemcpyAsync((T*)v + cut[q], (const T*)c.io->in_host[1] + cut[q], bytes, cudaMemcpyHostToDevice, c.io->cin));
+      GP_CUDA_OK(cudaMemcpyAsync((T*)xi + cut[q], (const T*)c.io->in_host[0] + cut[q], bytes, cudaMemcpyHostToDevice, c.io->cin));
+      arrived[q] = bag.make();
+      if (!arrived[q]) return GP_ERR_CUDA;
+      GP_CUDA_OK(cudaEventRecord(arrived[q], c.io->cin));
+    }
+    GP_CUDA_OK(cudaMemcpyAsync((T*)vbar, c.io->in_host[2], (size_t)n * sizeof(T), cudaMemcpyHostToDevice, c.io->cin));
+    vbar_arrived = bag.make();
+    if (!vbar_arrived) return GP_ERR_CUDA;
+    GP_CUDA_OK(cudaEventRecord(vbar_arrived, c.io->cin));
+  }
   // the head factorisation does not depend on the cotangents: side stream, overlapped with the reverse sweep
   SideStream* side = nullptr;
   GP_OK_OR_RETURN(side_stream(&side));
@@ -543,18 +584,31 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
     hc.st = side->stream;
     GP_OK_OR_RETURN(head_factor(hc, nullptr, 2 * (int)n0, true));
   }
-  if (spec) GP_OK_OR_RETURN(grad_pack<T>(c, v));
   GP_OK_OR_RETURN(ktime_begin(c.st));
-  bool flowed = false;
-  if constexpr (std::is_same<T, float>::value) {
-    if (spec && !(c.g->flags & GP_FLAG_PER_BATCH_LAUNCH)) {
+  if (flow) {
+    if constexpr (std::is_same<T, float>::value) {
+      for (int q = 0; q < chunks; ++q) {
+        if (c.io) GP_CUDA_OK(cudaStreamWaitEvent(c.st, arrived[q], 0));
+        grad_pack_kernel<T><<<(unsigned)((cut[q + 1] - cut[q] + 255) / 256), 256, 0, c.st>>>(
+            (const T*)c.g->x + cut[q] * c.g->d, v + cut[q], (Rec<T>*)c.rec() + cut[q], cut[q + 1] - cut[q], c.g->d);
+        GP_LAUNCH_CHECK();
 #define X(K, D) \
-      if (!flowed && c.g->k == K && c.g->d == D) { GP_OK_OR_RETURN((launch_vjp_flow<K, D>(c, xi, gbar, xibar))); flowed = true; }
-      GP_GRAD_PK_TABLE(X)
+        if (c.g->k == K && c.g->d == D) GP_OK_OR_RETURN((launch_vjp_geom<K, D>(c, xi, cut[q] < n0 ? n0 : cut[q], cut[q + 1])));
+        GP_GRAD_PK_TABLE(X)
 #undef X
+      }
+      if (c.io) GP_CUDA_OK(cudaStreamWaitEvent(c.st, vbar_arrived, 0));
+      GP_CUDA_OK(cudaMemcpyAsync(gbar, vbar, (size_t)n * sizeof(T), cudaMemcpyDeviceToDevice, c.st));
+      if (c.g->k == 8) GP_OK_OR_RETURN((launch_vjp_scatter<8>(c, gbar, xibar)));
+      else GP_OK_OR_RETURN((launch_vjp_scatter<16>(c, gbar, xibar)));
     }
-  }
-  if (!flowed) {
+  } else {
+    if (c.io) {
+      GP_CUDA_OK(cudaStreamWaitEvent(c.st, arrived[0], 0));
+      GP_CUDA_OK(cudaStreamWaitEvent(c.st, vbar_arrived, 0));
+    }
+    GP_CUDA_OK(cudaMemcpyAsync(gbar, vbar, (size_t)n * sizeof(T), cudaMemcpyDeviceToDevice, c.st));
+    if (spec) GP_OK_OR_RETURN(grad_pack<T>(c, v));
     const int64_t* off = c.g->batch_off;
     for (int b = c.g->n_batches - 1; b >= 0; --b)
       GP_OK_OR_RETURN((launch_grad_range<T, GRAD_VJP>(c, spec, v, xi, gbar, xibar, off[b], off[b + 1])));
@@ -564,6 +618,7 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
   if (n0 > 0) GP_OK_OR_RETURN(head_vjp(c, xi, gbar, xibar, &c.ctrl()->acc[3]));
   finalize_grad_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), 3, 4, 1.0 / c.kern->ell, thetabar);
   GP_LAUNCH_CHECK();
+  if (c.io) GP_CUDA_OK(cudaMemcpyAsync(c.io->out_host, xibar, (size_t)n * sizeof(T), cudaMemcpyDeviceToHost, c.st));
   return GP_OK;
 }
 
