@@ -282,6 +282,29 @@ def vjp(x, kern: Kernel, xi, v, vbar, *, n0=0, k=0, nbr=None, rowptr=None, col=N
     return xibar, tb
 
 
+def jvp(x, kern: Kernel, xi, v, dxi, dsigma, dell, *, n0=0, k=0, nbr=None, rowptr=None, col=None, batch_off=None) -> np.ndarray:
+    """JVP of forward along (dxi, dsigma, dell) at (xi, v = forward(xi)): returns dv [n]."""
+    args, keep, n = _graph_args(x, n0, k, nbr, rowptr, col, batch_off)
+    xi, v, dxi = _f64(xi), _f64(v), _f64(dxi)
+    dv = np.empty(n, dtype=np.float64)
+    kc = kern.c()
+    _check(lib().orc_jvp(*args, C.byref(kc), _p(xi, C.c_double), _p(v, C.c_double), _p(dxi, C.c_double),
+                         C.c_double(dsigma), C.c_double(dell), _p(dv, C.c_double)))
+    return dv
+
+
+def inverse_vjp(x, kern: Kernel, v, xi, h, *, n0=0, k=0, nbr=None, rowptr=None, col=None):
+    """VJP of inverse for a cotangent h on xi at (v, xi = inverse(v)): returns (v_bar [n], theta_bar [2])."""
+    args, keep, n = _graph_args(x, n0, k, nbr, rowptr, col, None)
+    v, xi, h = _f64(v), _f64(xi), _f64(h)
+    vbar = np.empty(n, dtype=np.float64)
+    tb = np.zeros(2, dtype=np.float64)
+    kc = kern.c()
+    _check(lib().orc_inverse_vjp(*args, C.byref(kc), _p(v, C.c_double), _p(xi, C.c_double), _p(h, C.c_double),
+                                 _p(vbar, C.c_double), _p(tb, C.c_double)))
+    return vbar, tb
+
+
 def cond_std(x, kern: Kernel, *, n0=0, k=0, nbr=None, rowptr=None, col=None) -> np.ndarray:
     """s_i of Eq. 2 for every point (head: diagonal of the dense factor): dv_i / dxi_i."""
     args, keep, n = _graph_args(x, n0, k, nbr, rowptr, col, None)

@@ -27,7 +27,7 @@
 // neighbour invariants (P-4), k=1 closed form (P-5), sigma scaling (P-6), power-of-two scale
 // invariance (P-7), 1-d Markov exponential closed form (P-8), logdet monotonicity (P-9),
 // order worked examples and k-d invariants (P-11), depth sequential = parallel (P-12),
-// long-double agreement (P-14).  Nothing is "parity unpinned" except absolute fp32 values
+// long-double agreement (P-14), JVP and inverse-VJP against central differences and against the VJP by duality (P-15).  Nothing is "parity unpinned" except absolute fp32 values
 // at N >= 2^24, which no formula in the paper fixes.
 #include <algorithm>
 #include <cmath>
@@ -457,6 +457,168 @@ int vjp_impl(const double* x, int d, const Graph& g, const Batches& B, const orc
   return bad ? 3 : 0;
 }
 
+// dK_ab/dtheta along the direction (dsigma, dell):  dK = dsigma 2K/sigma + dell sigma^2 drho/dell(r_ab) (zero on the diagonal
+// for the ell part: the nugget is relative, K_aa = sigma^2 (1 + eps)).
+template <class T>
+inline T dkappa_pair(const double* x, int d, const orc_kernel& kp, int64_t a, int64_t b, T dsig, T dell) {
+  T out = dsig * T(2) * kappa_pair<T>(x, d, kp, a, b) / T(kp.sigma);
+  if (a != b) {
+    T r = std::sqrt(T(d2_canon(x + a * d, x + b * d, d)));
+    out += dell * T(kp.sigma) * T(kp.sigma) * drho_dell<T>(kp.kind, r, T(kp.ell));
+  }
+  return out;
+}
+
+// Forward-mode derivative of the dense factor (textbook): K0 = L L^T, dK0 given => dL = L Phi(L^-1 dK0 L^-T), Phi = lower
+// triangle with the diagonal halved.  dK (n0 x n0, full symmetric, row-major) is overwritten by dL (lower part).
+template <class T>
+void chol_forward_mode(const T* L, int64_t n0, T* dK) {
+  // W = L^-1 dK  (column by column), then Z = W L^-T  (row by row: L^-1 applied to the rows), then Phi, then dL = L Phi
+  std::vector<T> colv(n0);
+  for (int64_t q = 0; q < n0; ++q) {
+    for (int64_t p = 0; p < n0; ++p) colv[p] = dK[p * n0 + q];
+    solve_lower<T>(L, n0, colv.data());
+    for (int64_t p = 0; p < n0; ++p) dK[p * n0 + q] = colv[p];
+  }
+  for (int64_t p = 0; p < n0; ++p) solve_lower<T>(L, n0, &dK[p * n0]);      // row p: (W L^-T)[p][:] = L^-1 W[p][:]^T
+  for (int64_t p = 0; p < n0; ++p)
+    for (int64_t q = 0; q < n0; ++q) dK[p * n0 + q] = (q < p) ? dK[p * n0 + q] : (q == p ? T(0.5) * dK[p * n0 + q] : T(0));
+  std::vector<T> out(size_t(n0) * n0, T(0));
+  for (int64_t p = 0; p < n0; ++p)
+    for (int64_t q = 0; q <= p; ++q) {
+      T sum = 0;
+      for (int64_t t = q; t <= p; ++t) sum += L[p * n0 + t] * dK[t * n0 + q];
+      out[p * n0 + q] = sum;
+    }
+  std::memcpy(dK, out.data(), sizeof(T) * size_t(n0) * n0);
+}
+
+// JVP of the forward map (xi, sigma, ell) -> v along (dxi, dsigma, dell)  ("forward ... derivatives";
+// DESIGN.md R-14).  Differentials of Eq. 2 with w = K_cc^-1 K_ci, alpha = K_cc^-1 v_c, u = (-w, 1):
+//   dm = u^T dK [alpha; 0] + w . dv_c,    d(s^2) = u^T dK u,    dv_i = dm + d(s^2) xi_i / (2 s) + s dxi_i.
+// Dense head: v_h = L0 xi_h  =>  dv_h = dL0 xi_h + L0 dxi_h.
+template <class T>
+int jvp_impl(const double* x, int d, const Graph& g, const Batches& B, const orc_kernel& kp, const double* xi,
+             const double* v, const double* dxi, double dsig, double dell, double* dv) {
+  int bad = 0;
+  if (!g.ragged() && g.n0 > 0) {
+    int64_t n0 = g.n0;
+    std::vector<T> L0;
+    if (head_factor<T>(x, d, kp, n0, L0)) return 3;
+    std::vector<T> dL(size_t(n0) * n0);
+    for (int64_t a = 0; a < n0; ++a)
+      for (int64_t b = 0; b < n0; ++b) dL[a * n0 + b] = dkappa_pair<T>(x, d, kp, a, b, T(dsig), T(dell));
+    chol_forward_mode<T>(L0.data(), n0, dL.data());
+    for (int64_t a = 0; a < n0; ++a) {
+      T sum = 0;
+      for (int64_t b = 0; b <= a; ++b) sum += dL[a * n0 + b] * T(xi[b]) + L0[a * n0 + b] * T(dxi[b]);
+      dv[a] = double(sum);
+    }
+  }
+  for (int64_t b = 0; b < B.count(); ++b) {
+    int64_t lo = B.lo(b), hi = B.hi(b);
+#pragma omp parallel if (hi - lo > 64)
+    {
+      Cond<T> C;
+      std::vector<T> alpha, u;
+#pragma omp for schedule(static)
+      for (int64_t i = lo; i < hi; ++i) {
+        const int32_t* c; int m;
+        g.row(i, c, m);
+        if (C.run(x, d, kp, i, c, m)) {
+#pragma omp atomic write
+          bad = 1;
+          dv[i] = NAN;
+          continue;
+        }
+        T s = std::sqrt(C.s2);
+        alpha.resize(m + 1); u.resize(m + 1);
+        for (int a = 0; a < m; ++a) { alpha[a] = T(v[c[a]]); u[a] = -C.w[a]; }
+        C.solve_kcc(alpha.data());
+        alpha[m] = 0; u[m] = 1;
+        T dm = 0, ds2 = 0;
+        for (int a = 0; a <= m; ++a)
+          for (int bb = 0; bb <= m; ++bb) {
+            int64_t pa = (a < m) ? c[a] : i, pb = (bb < m) ? c[bb] : i;
+            T dk = dkappa_pair<T>(x, d, kp, pa, pb, T(dsig), T(dell));
+            dm += u[a] * dk * alpha[bb];
+            ds2 += u[a] * dk * u[bb];
+          }
+        for (int a = 0; a < m; ++a) dm += C.w[a] * T(dv[c[a]]);
+        dv[i] = double(dm + ds2 * T(xi[i]) / (T(2) * s) + s * T(dxi[i]));
+      }
+    }
+  }
+  return bad ? 3 : 0;
+}
+
+// VJP of the inverse map (v, sigma, ell) -> xi for a cotangent xi_bar = h  (R-14):
+//   xi_i = (v_i - w . v_c) / s:   v_bar_i += h_i / s,   v_bar_c -= (h_i / s) w,
+//   K_bar = -(h_i / s) u [alpha; 0]^T - (h_i xi_i / (2 s^2)) u u^T,   theta_bar += sum_ab K_bar_ab dK_ab/dtheta.
+// No sweep is needed: every point contributes independently.  Dense head: xi_h = L0^-1 v_h =>
+// v_bar_h += L0^-T h_h and, parameter by parameter, theta_bar_p -= h_h . L0^-1 dL0_p xi_h (forward mode of the factor).
+template <class T>
+int inverse_vjp_impl(const double* x, int d, const Graph& g, const orc_kernel& kp, const double* v, const double* xi,
+                     const double* h, double* vbar, double* thetabar) {
+  std::vector<long double> acc(g.n, 0.0L);
+  long double ts = 0, tl = 0;
+  int bad = 0;
+  int64_t first = g.first();
+  if (!g.ragged() && g.n0 > 0) {
+    int64_t n0 = g.n0;
+    std::vector<T> L0, y(n0);
+    if (head_factor<T>(x, d, kp, n0, L0)) return 3;
+    for (int64_t a = 0; a < n0; ++a) y[a] = T(h[a]);
+    solve_lower_t<T>(L0.data(), n0, y.data());                 // L0^-T h_h
+    for (int64_t a = 0; a < n0; ++a) acc[a] += (long double)y[a];
+    for (int p = 0; p < 2; ++p) {
+      std::vector<T> dL(size_t(n0) * n0);
+      for (int64_t a = 0; a < n0; ++a)
+        for (int64_t b = 0; b < n0; ++b) dL[a * n0 + b] = dkappa_pair<T>(x, d, kp, a, b, T(p == 0), T(p == 1));
+      chol_forward_mode<T>(L0.data(), n0, dL.data());
+      std::vector<T> t(n0);
+      for (int64_t a = 0; a < n0; ++a) {
+        T sum = 0;
+        for (int64_t b = 0; b <= a; ++b) sum += dL[a * n0 + b] * T(xi[b]);
+        t[a] = sum;
+      }
+      solve_lower<T>(L0.data(), n0, t.data());                 // L0^-1 dL0 xi_h
+      long double dot = 0;
+      for (int64_t a = 0; a < n0; ++a) dot += (long double)(T(h[a]) * t[a]);
+      (p == 0 ? ts : tl) -= dot;
+    }
+  }
+  // sequential over points (deterministic scatter); the per-point work is the oracle's usual conditioning
+  Cond<T> C;
+  std::vector<T> alpha, u;
+  for (int64_t i = first; i < g.n; ++i) {
+    const int32_t* c; int m;
+    g.row(i, c, m);
+    if (C.run(x, d, kp, i, c, m)) { bad = 1; continue; }
+    T s = std::sqrt(C.s2), hs = T(h[i]) / s;
+    acc[i] += (long double)hs;
+    alpha.resize(m + 1); u.resize(m + 1);
+    for (int a = 0; a < m; ++a) { alpha[a] = T(v[c[a]]); u[a] = -C.w[a]; acc[c[a]] -= (long double)(hs * C.w[a]); }
+    C.solve_kcc(alpha.data());
+    alpha[m] = 0; u[m] = 1;
+    T coef = T(h[i]) * T(xi[i]) / (T(2) * C.s2);
+    T qs = 0, ql = 0;
+    for (int a = 0; a <= m; ++a)
+      for (int bb = 0; bb <= m; ++bb) {
+        T kbar = -hs * u[a] * alpha[bb] - coef * u[a] * u[bb];
+        int64_t pa = (a < m) ? c[a] : i, pb = (bb < m) ? c[bb] : i;
+        qs += kbar * dkappa_pair<T>(x, d, kp, pa, pb, T(1), T(0));
+        ql += kbar * dkappa_pair<T>(x, d, kp, pa, pb, T(0), T(1));
+      }
+    ts += (long double)qs;
+    tl += (long double)ql;
+  }
+  for (int64_t i = 0; i < g.n; ++i) vbar[i] = double(acc[i]);
+  thetabar[0] = double(ts);
+  thetabar[1] = double(tl);
+  return bad ? 3 : 0;
+}
+
 // ---- order ---------------------------------------------------------------------------
 inline int level_of(int64_t i) {  // floor(log2(i+1))
   int l = 0;
@@ -664,6 +826,18 @@ int orc_vjp(ORC_GRAPH_ARGS, const orc_kernel* kp, const double* xi, const double
   ORC_MAKE_GRAPH
   return use_long_double ? vjp_impl<long double>(x, d, g, B, *kp, xi, v, vbar, xibar, thetabar2)
                          : vjp_impl<double>(x, d, g, B, *kp, xi, v, vbar, xibar, thetabar2);
+}
+
+int orc_jvp(ORC_GRAPH_ARGS, const orc_kernel* kp, const double* xi, const double* v, const double* dxi, double dsigma,
+            double dell, double* dv) {
+  ORC_MAKE_GRAPH
+  return jvp_impl<double>(x, d, g, B, *kp, xi, v, dxi, dsigma, dell, dv);
+}
+int orc_inverse_vjp(ORC_GRAPH_ARGS, const orc_kernel* kp, const double* v, const double* xi, const double* h, double* vbar,
+                    double* thetabar2) {
+  ORC_MAKE_GRAPH
+  (void)B;
+  return inverse_vjp_impl<double>(x, d, g, *kp, v, xi, h, vbar, thetabar2);
 }
 
 }  // extern "C"

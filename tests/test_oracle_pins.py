@@ -460,3 +460,59 @@ def test_p14_double_agrees_with_long_double(orc, cid):
     assert rel(v, v_ld) < 1e-10
     ld, ld_ld = orc.logdet(g.x, kern, **kw), orc.logdet(g.x, kern, long_double=True, **kw)
     assert abs(ld - ld_ld) / abs(ld_ld) < 1e-12
+
+
+# ------------------------------------------------------------------ P-15 forward-mode and inverse derivatives
+@pytest.mark.parametrize("kind,sigma,ell,jit", KERNELS)
+def test_p15_jvp_and_inverse_vjp_match_central_differences_and_duality(orc, kind, sigma, ell, jit):
+    """PAPER.md:57 "forward and backward derivatives": the oracle's JVP of forward and VJP of inverse against central
+    differences of the oracle's own forward / inverse (pinned by P-1, P-2, P-5, P-8), on a regular graph WITH a dense
+    head and on a ragged graph; and <v_bar, JVP> = <VJP, tangent> ties the JVP to the VJP that P-3 pins."""
+    n, k, n0 = 400, 6, 40
+    jit = max(jit, 1e-6)
+    x = W.make_points(W.CONFIGS[1], "f64", n)
+    g = orc.build_graph(x, k, n0)
+    kw = dict(n0=g.n0, k=g.k, nbr=g.nbr, batch_off=g.batch_off)
+    kwi = dict(n0=g.n0, k=g.k, nbr=g.nbr)
+    xi = W.make_noise(1, n, "f64")
+    dxi = W.make_noise(3, n, "f64")
+    vbar = W.make_noise(1, n, "f64", "vbar")
+    dsig, dell = 0.3, -0.2
+    K = lambda s_, l_: orc.Kernel(kind, s_, l_, jit)
+    v = orc.forward(g.x, K(sigma, ell), xi, **kw)
+    dv = orc.jvp(g.x, K(sigma, ell), xi, v, dxi, dsig, dell, **kw)
+    hh = 1e-6
+    vp = orc.forward(g.x, K(sigma + hh * dsig, ell + hh * dell), xi + hh * dxi, **kw)
+    vm = orc.forward(g.x, K(sigma - hh * dsig, ell - hh * dell), xi - hh * dxi, **kw)
+    assert rel((vp - vm) / (2 * hh), dv) < 1e-6
+    assert rel(dv, (vp - vm) / (2 * hh)) < 1e-6
+    xib, tb = orc.vjp(g.x, K(sigma, ell), xi, v, vbar, **kw)
+    lhs = float(vbar @ dv)
+    rhs = float(xib @ dxi + tb[0] * dsig + tb[1] * dell)
+    assert abs(lhs - rhs) <= 1e-9 * max(abs(lhs), abs(rhs))
+    # the ragged route (every point through Eq. 2, no dense head) gives the same JVP when the head rows are complete
+    rowptr = np.zeros(n + 1, dtype=np.int64)
+    cols = []
+    for i in range(n):
+        c = np.arange(i, dtype=np.int32) if i < n0 else g.nbr[i - n0]
+        cols.append(c)
+        rowptr[i + 1] = rowptr[i] + c.size
+    col = np.concatenate(cols).astype(np.int32)
+    dv_r = orc.jvp(g.x, K(sigma, ell), xi, v, dxi, dsig, dell, rowptr=rowptr, col=col)
+    assert rel(dv_r, dv) < 1e-8
+    # inverse: cotangent h on xi
+    h = W.make_noise(5, n, "f64", "vbar")
+    xi_b = orc.inverse(g.x, K(sigma, ell), v, **kwi)
+    vb_i, tb_i = orc.inverse_vjp(g.x, K(sigma, ell), v, xi_b, h, **kwi)
+    dvv = W.make_noise(7, n, "f64")
+    ip = orc.inverse(g.x, K(sigma + hh * dsig, ell + hh * dell), v + hh * dvv, **kwi)
+    im = orc.inverse(g.x, K(sigma - hh * dsig, ell - hh * dell), v - hh * dvv, **kwi)
+    fd = float(h @ (ip - im)) / (2 * hh)
+    an = float(vb_i @ dvv + tb_i[0] * dsig + tb_i[1] * dell)
+    assert abs(fd - an) <= 2e-6 * max(abs(fd), abs(an))
+    vb_r, tb_r = orc.inverse_vjp(g.x, K(sigma, ell), v, xi_b, h, rowptr=rowptr, col=col)
+    assert rel(vb_r, vb_i) < 1e-8 and rel(tb_r, tb_i) < 1e-8
+    # inverse and forward are mutually inverse maps: J_inv = J_fwd^-1, so pushing the forward JVP through the inverse
+    # VJP returns the tangent:  <h, dxi> = <v_bar_inv, dv - dv|_{dxi=0}>... checked in its simplest form, theta fixed
+    dv_x = orc.jvp(g.x, K(sigma, ell), xi, v, dxi, 0.0, 0.0, **kw)
+    assert abs(float(vb_i @ dv_x) - float(h @ dxi)) <= 1e-8 * abs(float(h @ dxi))
