@@ -117,6 +117,21 @@ gp_status gp_logdet(const gp_graph* g, const gp_kernel* kern, double* logdet_dev
 gp_status gp_vjp(const gp_graph* g, const gp_kernel* kern, const void* xi, const void* v, const void* v_bar,
                  void* xi_bar, double* theta_bar_dev, void* ws, size_t ws_bytes, void* cuda_stream);
 
+/* Forward-mode derivative of gp_forward ("forward ... derivatives"): at the point (xi, v = forward(xi; theta))
+ * and along the tangent (xi_dot [n], sigma_dot, ell_dot) returns v_dot [n] = d forward.  xi, v, xi_dot: device [n] (in);
+ * v_dot: device [n] (out).  <v_bar, v_dot> = <xi_bar, xi_dot> + theta_bar . (sigma_dot, ell_dot) with gp_vjp's outputs.
+ * Workspace: gp_workspace_bytes(g, GP_OP_VJP).                                                                       */
+gp_status gp_jvp(const gp_graph* g, const gp_kernel* kern, const void* xi, const void* v, const void* xi_dot, double sigma_dot,
+                 double ell_dot, void* v_dot, void* ws, size_t ws_bytes, void* cuda_stream);
+
+/* VJP of gp_inverse ("kernel parameter derivatives"): at (v, xi = inverse(v; theta)) and for a
+ * cotangent xi_bar [n] on xi returns v_bar [n] and theta_bar = (d/dsigma, d/dell) of <xi_bar, inverse(v; theta)>.
+ * Every point contributes independently (no sweep); v_bar is accumulated with floating-point atomics.
+ * v, xi, xi_bar: device [n] (in);  v_bar: device [n] (out);  theta_bar_dev: device double[2] (out).
+ * Workspace: gp_workspace_bytes(g, GP_OP_VJP).  (The gradient of the log-determinant is gp_logdet's second output.)   */
+gp_status gp_inverse_vjp(const gp_graph* g, const gp_kernel* kern, const void* v, const void* xi, const void* xi_bar,
+                         void* v_bar, double* theta_bar_dev, void* ws, size_t ws_bytes, void* cuda_stream);
+
 /* Multi-sample apply: S = n_samples noise vectors on one graph and one set of kernel parameters (MGVI /
  * geoVI "require the forward pass for posterior sampling").  The conditioning of Eq. 2 - K, its
  * factor, the weights and s - is computed once per point and applied to every sample.  xi, v: device [n][S], row-major

@@ -26,7 +26,7 @@ KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
 EXPORTS = ["gp_workspace_bytes", "gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host",
            "gp_inverse_host", "gp_logdet_host", "gp_vjp_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
            "gp_check_errors", "gp_status_string", "gp_has_specialised", "gp_launch_count", "gp_kernel_time_enable",
-           "gp_kernel_time_last", "gp_measure_alu_peak", "gp_workspace_bytes_multi", "gp_forward_multi", "gp_inverse_multi"]
+           "gp_kernel_time_last", "gp_measure_alu_peak", "gp_workspace_bytes_multi", "gp_forward_multi", "gp_inverse_multi", "gp_jvp", "gp_inverse_vjp"]
 
 
 class GraphGPError(RuntimeError):
@@ -83,6 +83,10 @@ def lib():
                                      vp, vp, vp, C.c_int32, C.POINTER(C.c_int32), vp, sz, vp]
         L.gp_graph_build_times.argtypes = [vp, vp]
         L.gp_check_errors.argtypes = [vp, C.POINTER(C.c_int64)]
+        L.gp_jvp.argtypes = gk + [vp, vp, vp, C.c_double, C.c_double, vp, vp, sz, vp]
+        L.gp_inverse_vjp.argtypes = gk + [vp, vp, vp, vp, vp, vp, sz, vp]
+        L.gp_jvp.restype = C.c_int
+        L.gp_inverse_vjp.restype = C.c_int
         L.gp_workspace_bytes_multi.restype = C.c_size_t
         L.gp_workspace_bytes_multi.argtypes = [C.POINTER(_Graph), C.c_int32, C.c_int32]
         L.gp_forward_multi.argtypes = gk + [C.c_int32, vp, vp, vp, sz, vp]
@@ -317,6 +321,31 @@ def gp_vjp(graph: Graph, kern: Kernel, xi, v, v_bar, stream=None):
     _check(lib().gp_vjp(C.byref(g), C.byref(k), xi.data_ptr(), v.data_ptr(), v_bar.data_ptr(), xi_bar.data_ptr(),
                         tb.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "gp_vjp")
     return xi_bar, tb
+
+
+def gp_jvp(graph: Graph, kern: Kernel, xi, v, xi_dot, sigma_dot: float, ell_dot: float, stream=None):
+    """Forward-mode derivative of gp_forward: v_dot [n] along (xi_dot, sigma_dot, ell_dot) at (xi, v)."""
+    torch = _torch()
+    _vec(graph, xi, "xi"), _vec(graph, v, "v"), _vec(graph, xi_dot, "xi_dot")
+    v_dot = torch.empty_like(xi)
+    ws = graph.workspace(GP_OP_VJP)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_jvp(C.byref(g), C.byref(k), xi.data_ptr(), v.data_ptr(), xi_dot.data_ptr(), float(sigma_dot),
+                        float(ell_dot), v_dot.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "gp_jvp")
+    return v_dot
+
+
+def gp_inverse_vjp(graph: Graph, kern: Kernel, v, xi, xi_bar, stream=None):
+    """VJP of gp_inverse: (v_bar [n], theta_bar double[2]) for a cotangent xi_bar at (v, xi = inverse(v))."""
+    torch = _torch()
+    _vec(graph, v, "v"), _vec(graph, xi, "xi"), _vec(graph, xi_bar, "xi_bar")
+    v_bar = torch.empty_like(v)
+    tb = torch.empty(2, dtype=torch.float64, device=graph.x.device)
+    ws = graph.workspace(GP_OP_VJP)
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_inverse_vjp(C.byref(g), C.byref(k), v.data_ptr(), xi.data_ptr(), xi_bar.data_ptr(), v_bar.data_ptr(),
+                                tb.data_ptr(), ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "gp_inverse_vjp")
+    return v_bar, tb
 
 
 def _multi(graph: Graph, kern: Kernel, op: int, name: str, src, out, stream):

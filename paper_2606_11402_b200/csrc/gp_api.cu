@@ -176,6 +176,22 @@ gp_status gp_vjp(const gp_graph* g, const gp_kernel* kern, const void* xi, const
   return run_vjp(c, xi, v, v_bar, xi_bar, theta_bar_dev);
 }
 
+gp_status gp_jvp(const gp_graph* g, const gp_kernel* kern, const void* xi, const void* v, const void* xi_dot, double sigma_dot,
+                 double ell_dot, void* v_dot, void* ws, size_t ws_bytes, void* cuda_stream) {
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_VJP, ws, ws_bytes, cuda_stream, &c));
+  if (!xi || !v || !xi_dot || !v_dot) return GP_ERR_INVALID_ARG;
+  return run_jvp(c, xi, v, xi_dot, sigma_dot, ell_dot, v_dot);
+}
+
+gp_status gp_inverse_vjp(const gp_graph* g, const gp_kernel* kern, const void* v, const void* xi, const void* xi_bar,
+                         void* v_bar, double* theta_bar_dev, void* ws, size_t ws_bytes, void* cuda_stream) {
+  OpCtx c;
+  GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_VJP, ws, ws_bytes, cuda_stream, &c));
+  if (!xi || !v || !xi_bar || !v_bar || !theta_bar_dev) return GP_ERR_INVALID_ARG;
+  return run_inverse_vjp(c, v, xi, xi_bar, v_bar, theta_bar_dev);
+}
+
 gp_status gp_forward_host(const gp_graph* g, const gp_kernel* kern, const void* xi_host, void* v_host, void* in_dev,
                           void* out_dev, void* ws, size_t ws_bytes, void* cuda_stream) {
   if (!g || !xi_host || !v_host || !in_dev || !out_dev) return GP_ERR_INVALID_ARG;

@@ -202,9 +202,9 @@ inline WsLayout ws_layout(const gp_graph* g, int op) {
   w.rec_off = off; off += align_up(n * 4 * B, 256);
   w.g_off = off;
   if (op == GP_OP_VJP) off += align_up(n * B, 256);
-  // two-phase VJP (fp32): per conditioned point the k weights and {s, A_i, B_i, ok}
+  // per conditioned point the k weights and {s, A_i, B_i, ok} (two-phase VJP, JVP, inverse VJP), working dtype
   w.wbuf_off = off;
-  if (op == GP_OP_VJP && g->dtype == GP_F32) off += align_up((n - n0) * ((size_t)g->k + 4) * sizeof(float), 256);
+  if (op == GP_OP_VJP) off += align_up((n - n0) * ((size_t)g->k + 4) * B, 256);
   w.total = off;
   return w;
 }
@@ -295,6 +295,12 @@ gp_status run_inverse(const OpCtx& c, const void* v, void* xi);
 gp_status run_logdet(const OpCtx& c, double* logdet, double* grad);
 gp_status run_vjp(const OpCtx& c, const void* xi, const void* v, const void* vbar, void* xibar, double* thetabar);
 gp_status run_logdet_grad(const OpCtx& c);   // conditioning part of d logdet / d ell into ctrl->acc[2]
+// gp_vjp.cu: packs the records and writes, for every point i >= n0, the k weights w = K_cc^-1 K_ci (wbuf [n - n0][k]) and
+// {s (unit sigma), A_i = ell dv_i/dell, B_i = dv_i/dsigma, ok} (sab [n - n0][4], after the weights), all in the working dtype
+gp_status run_geometry(const OpCtx& c, const void* xi, const void* v);
+// gp_jvp.cu
+gp_status run_jvp(const OpCtx& c, const void* xi, const void* v, const void* xi_dot, double sigma_dot, double ell_dot, void* v_dot);
+gp_status run_inverse_vjp(const OpCtx& c, const void* v, const void* xi, const void* xi_bar, void* v_bar, double* theta_bar);
 bool has_specialised(int dtype, int k, int d, int kind);
 
 }  // namespace gp

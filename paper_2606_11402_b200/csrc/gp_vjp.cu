@@ -364,6 +364,60 @@ __global__ void grad_generic_kernel(const T* __restrict__ x, const T* __restrict
   block_atomic_add(acc_ell, &ctrl->acc[MODE == GRAD_VJP ? 4 : 2], red);
 }
 
+// ---- generic geometry kernel: what vjp_geom_kernel writes, for any (k, d, kind, dtype) ---------------------------------
+// w = K_cc^-1 K_ci, s, A_i = y[0:k].alpha + sigma xi_i (y.u) / (2 s) (= ell dv_i/dell at fixed v_c), B_i = s xi_i
+template <typename T>
+__global__ void geom_generic_kernel(const T* __restrict__ x, const T* __restrict__ vals, const int32_t* __restrict__ nbr,
+                                    const T* __restrict__ xi, T* __restrict__ wbuf, T* __restrict__ sab, int64_t n0,
+                                    int64_t n, int d, int k, int kind, KParams<T> kp, Control* ctrl, int active) {
+  extern __shared__ double smem_raw[];
+  const int tid = threadIdx.x;
+  const int64_t i = n0 + (int64_t)blockIdx.x * active + tid;
+  if (tid >= active || i >= n) return;
+  Scratch<T> A{reinterpret_cast<T*>(smem_raw) + tid, active};
+  const int32_t* row = nbr + (i - n0) * k;
+  const int NT = (k + 1) * (k + 2) / 2;
+  Cond<T> c = condition_generic<T>(x, vals, d, k, kind, row, i, kp, A);
+  for (int j = k - 1; j >= 0; --j) {        // back-substitution: A[k][j] <- w_j, A[NT + j] <- alpha_j
+    T w = A[tri(k, j)], a = A[NT + j];
+    for (int r = j + 1; r < k; ++r) {
+      T lrj = A[tri(r, j)];
+      w = Math<T>::fma(-lrj, A[tri(k, r)], w);
+      a = Math<T>::fma(-lrj, A[NT + r], a);
+    }
+    T inv = T(1) / A[tri(j, j)];
+    A[tri(k, j)] = w * inv;
+    A[NT + j] = a * inv;
+  }
+  const int YO = NT + k;
+  for (int j = 0; j <= k; ++j) A[YO + j] = T(0);
+  for (int r = 1; r <= k; ++r) {            // y = (ell dM/dell) u, u = (-w, 1)
+    int64_t pr = (r == k) ? i : (int64_t)row[r];
+    T ur = (r == k) ? T(1) : -A[tri(k, r)];
+    T yr = T(0);
+    for (int cc = 0; cc < r; ++cc) {
+      T dq = drho_rt<T>(kind, dist_q<T>(x, d, pr, (int64_t)row[cc], kp.qscale));
+      yr = Math<T>::fma(-dq, A[tri(k, cc)], yr);
+      A[YO + cc] = Math<T>::fma(dq, ur, A[YO + cc]);
+    }
+    A[YO + r] += yr;
+  }
+  T yu = A[YO + k], ya = T(0);
+  for (int j = 0; j < k; ++j) {
+    yu = Math<T>::fma(-A[YO + j], A[tri(k, j)], yu);
+    ya = Math<T>::fma(A[YO + j], A[NT + j], ya);
+  }
+  if (!c.ok) atomicAdd(&ctrl->n_bad, 1ULL);
+  T* wrow = wbuf + (i - n0) * k;
+  for (int j = 0; j < k; ++j) wrow[j] = A[tri(k, j)];
+  const T xi_i = xi[i];
+  T* o = sab + (i - n0) * 4;
+  o[0] = c.s;
+  o[1] = ya + T(0.5) * kp.sigma * xi_i * yu / c.s;
+  o[2] = c.s * xi_i;
+  o[3] = c.ok ? T(1) : T(0);
+}
+
 // ---- host side --------------------------------------------------------------------------------------------
 int generic_active_threads(int k, size_t elem_bytes, bool with_vjp);   // gp_ops.cu
 
@@ -620,6 +674,44 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
   GP_LAUNCH_CHECK();
   if (c.io) GP_CUDA_OK(cudaMemcpyAsync(c.io->out_host, xibar, (size_t)n * sizeof(T), cudaMemcpyDeviceToHost, c.st));
   return GP_OK;
+}
+
+template <typename T>
+static gp_status geometry_t(const OpCtx& c, const T* xi, const T* v) {
+  const int64_t n = c.g->n, n0 = c.g->n0, cnt = n - n0;
+  if (cnt <= 0) return GP_OK;
+  if constexpr (std::is_same<T, float>::value) {
+    if (grad_use_spec(c)) {
+      bool pk = false;
+#define X(K, D) \
+      if (c.g->k == K && c.g->d == D) pk = true;
+      GP_GRAD_PK_TABLE(X)
+#undef X
+      if (pk) {
+        GP_OK_OR_RETURN(grad_pack<T>(c, v));
+#define X(K, D) \
+        if (c.g->k == K && c.g->d == D) return launch_vjp_geom<K, D>(c, xi, n0, n);
+        GP_GRAD_PK_TABLE(X)
+#undef X
+      }
+    }
+  }
+  const int k = c.g->k;
+  int active = generic_active_threads(k, sizeof(T), true);
+  int threads = (active + 31) / 32 * 32;
+  size_t smem = (size_t)generic_scratch_elems(k, true) * sizeof(T) * active;
+  GP_CUDA_OK(cudaFuncSetAttribute(geom_generic_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024));
+  unsigned grid = (unsigned)((cnt + active - 1) / active);
+  KParams<T> kp = make_kparams<T>(*c.kern);
+  T* wbuf = (T*)c.wbuf();
+  geom_generic_kernel<T><<<grid, threads, smem, c.st>>>((const T*)c.g->x, v, c.g->nbr, xi, wbuf, wbuf + (size_t)cnt * k, n0, n,
+                                                       c.g->d, k, c.kern->kind, kp, c.ctrl(), active);
+  GP_LAUNCH_CHECK();
+  return GP_OK;
+}
+gp_status run_geometry(const OpCtx& c, const void* xi, const void* v) {
+  return c.g->dtype == GP_F64 ? geometry_t<double>(c, (const double*)xi, (const double*)v)
+                              : geometry_t<float>(c, (const float*)xi, (const float*)v);
 }
 
 gp_status run_vjp(const OpCtx& c, const void* xi, const void* v, const void* vbar, void* xibar, double* thetabar) {

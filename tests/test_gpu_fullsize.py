@@ -166,9 +166,41 @@ def test_config3_full_size_all_ops(gp, orc):
     assert (e_tb <= F32_GRAD).all(), (e_tb, tb_ref)
     assert e_xib <= F32_GRAD, e_xib
     # sampled one-step checks on the GPU's own v (forward) and its inverse
-    xi_back = gp.gp_inverse(G, c.K, v).cpu().numpy().astype(np.float64)
+    xi_back_d = gp.gp_inverse(G, c.K, v)
+    xi_back = xi_back_d.cpu().numpy().astype(np.float64)
     wv, wxi = sampled_one_step(orc, c, v_h, xi_back, 4096, 103)
     assert wv <= F32_V * v_ref.std() and wxi <= F32_V * v_ref.std(), (wv, wxi)
+    # multi-sample apply at full size: two noise vectors per call, column by column against the oracle
+    xi2_h = np.stack([c.xi_h, W.make_noise(13, c.n, "f32", "xi")], axis=1).copy()
+    v2 = gp.gp_forward_multi(G, c.K, torch.as_tensor(xi2_h, device="cuda")).cpu().numpy().astype(np.float64)
+    v2_ref = orc.forward(c.xg, c.okern(orc), xi2_h[:, 1].astype(np.float64), n0=cfg.n0, k=cfg.k, nbr=c.nbr, batch_off=G.batch_off)
+    assert np.abs(v2[:, 0] - v_ref).max() <= F32_V * v_ref.std()
+    assert np.abs(v2[:, 1] - v2_ref).max() <= F32_V * v2_ref.std()
+    # JVP of forward and VJP of inverse on the whole graph run; the oracle checks a 2^20 prefix of the graph order
+    # (itself a valid generation graph) because its inverse-VJP scatter is sequential
+    dxi_h = W.make_noise(23, c.n, "f32", "xi")
+    h_h = W.make_noise(33, c.n, "f32", "vbar")
+    dsig, dell = 0.3, -0.2 * cfg.ell
+    dv = gp.gp_jvp(G, c.K, torch.as_tensor(c.xi_h, device="cuda"), v, torch.as_tensor(dxi_h, device="cuda"), dsig, dell)
+    vbi, tbi = gp.gp_inverse_vjp(G, c.K, v, xi_back_d, torch.as_tensor(h_h, device="cuda"))
+    assert gp.check_errors(G.workspace(gp.GP_OP_VJP)) == 0
+    assert bool(torch.isfinite(dv).all()) and bool(torch.isfinite(vbi).all())
+    lhs = float((torch.as_tensor(vb_h, device="cuda").double() * dv.double()).sum().cpu())
+    rhs = float((torch.as_tensor(xib) * torch.as_tensor(dxi_h.astype(np.float64))).sum()) + float(tb[0].cpu()) * dsig + float(tb[1].cpu()) * dell
+    assert abs(lhs - rhs) <= F32_GRAD * max(abs(lhs), abs(rhs)), (lhs, rhs)        # duality at full size
+    M = 1 << 20
+    pb = np.unique(np.minimum(G.batch_off, M))
+    Gp = gp.Graph(x=G.x[:M].contiguous(), nbr=G.nbr[:M - cfg.n0].contiguous(), batch_off=pb, n0=cfg.n0)
+    dvp = gp.gp_jvp(Gp, c.K, torch.as_tensor(c.xi_h[:M], device="cuda"), v[:M].contiguous(), torch.as_tensor(dxi_h[:M], device="cuda"),
+                    dsig, dell).cpu().numpy().astype(np.float64)
+    dv_ref = orc.jvp(c.xg[:M], c.okern(orc), c.xi_h[:M].astype(np.float64), v_h[:M], dxi_h[:M].astype(np.float64), dsig, dell,
+                     n0=cfg.n0, k=cfg.k, nbr=c.nbr[:M - cfg.n0], batch_off=pb)
+    assert np.abs(dvp - dv_ref).max() <= F32_GRAD * np.abs(dv_ref).max()
+    vbp, tbp = gp.gp_inverse_vjp(Gp, c.K, v[:M].contiguous(), xi_back_d[:M].contiguous(), torch.as_tensor(h_h[:M], device="cuda"))
+    vb_ref, tbp_ref = orc.inverse_vjp(c.xg[:M], c.okern(orc), v_h[:M], xi_back[:M], h_h[:M].astype(np.float64), n0=cfg.n0, k=cfg.k,
+                                      nbr=c.nbr[:M - cfg.n0])
+    assert np.abs(vbp.cpu().numpy() - vb_ref).max() <= F32_GRAD * np.abs(vb_ref).max()
+    assert (np.abs(tbp.cpu().numpy() - tbp_ref) <= F32_GRAD * np.abs(tbp_ref)).all(), (tbp, tbp_ref)
 
 
 def test_config4_full_size(gp, orc):
