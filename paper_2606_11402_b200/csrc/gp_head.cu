@@ -256,7 +256,9 @@ static gp_status head_chol(const OpCtx& c, int n_carried, bool overlapped) {
   Control* ctrl = c.ctrl();
   void* args[] = {(void*)&A, (void*)&n0_arg, (void*)&rows_total, (void*)&ctrl};
   int ctas = grid_ctas;
-  if (overlapped) {                                         // a quarter of the SMs; more when many rows are carried
+  // beside a LONG bulk kernel the head takes a quarter of the SMs (more when many rows are carried) and is hidden;
+  // beside a short one (config 2: 2^20 points, 0.2 ms of bulk work) it is the critical path and takes every SM
+  if (overlapped && c.g->n - c.g->n0 >= ((int64_t)1 << (c.g->dtype == GP_F64 ? 19 : 22))) {
     ctas = n_carried > n0 ? grid_ctas / 2 : grid_ctas / 4;
     if (ctas < 1) ctas = 1;
   }
