@@ -41,7 +41,8 @@ extern "C" {
 typedef enum {
   GP_OK = 0,
   GP_ERR_INVALID_ARG = 1,
-  GP_ERR_UNSUPPORTED = 2, /* (k, d, dtype) outside what the library handles (k <= 64, d <= 4) */
+  GP_ERR_UNSUPPORTED = 2, /* (k, d, dtype) outside what the call handles: k <= 128, d <= 4 for forward / inverse /
+                             logdet and the builder; k <= 64 for the gradient, JVP and multi-sample calls */
   GP_ERR_NOT_PD = 3,
   GP_ERR_CUDA = 4,
   GP_ERR_WORKSPACE = 5 /* ws == NULL or ws_bytes < gp_workspace_bytes() */
@@ -76,7 +77,8 @@ typedef struct {
   int64_t n;         /* number of points N                                                            */
   int64_t n0;        /* size of the dense initial block (Alg. 1 line 1); k <= n0 <= n    */
   int32_t d;         /* spatial dimension, 1..4                                                        */
-  int32_t k;         /* neighbours per point, 1..64                                                    */
+  int32_t k;         /* neighbours per point, 1..128 (PAPER.md:53 sends k >~ 64 to JAX; here 64 < k <= 128 runs
+                        on warp-per-point fp64 kernels: forward, inverse, logdet only)                  */
   int32_t n_batches; /* L                                                                              */
   int32_t dtype;     /* gp_dtype of x, xi, v, v_bar, xi_bar                                            */
   int32_t flags;     /* GP_FLAG_*                                                                      */

@@ -173,6 +173,7 @@ gp_status gp_vjp(const gp_graph* g, const gp_kernel* kern, const void* xi, const
   OpCtx c;
   GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_VJP, ws, ws_bytes, cuda_stream, &c));
   if (!xi || !v || !v_bar || !xi_bar || !theta_bar_dev) return GP_ERR_INVALID_ARG;
+  if (g->k > kMaxKGrad) return GP_ERR_UNSUPPORTED;
   return run_vjp(c, xi, v, v_bar, xi_bar, theta_bar_dev);
 }
 
@@ -181,6 +182,7 @@ gp_status gp_jvp(const gp_graph* g, const gp_kernel* kern, const void* xi, const
   OpCtx c;
   GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_VJP, ws, ws_bytes, cuda_stream, &c));
   if (!xi || !v || !xi_dot || !v_dot) return GP_ERR_INVALID_ARG;
+  if (g->k > kMaxKGrad) return GP_ERR_UNSUPPORTED;
   return run_jvp(c, xi, v, xi_dot, sigma_dot, ell_dot, v_dot);
 }
 
@@ -189,6 +191,7 @@ gp_status gp_inverse_vjp(const gp_graph* g, const gp_kernel* kern, const void* v
   OpCtx c;
   GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_VJP, ws, ws_bytes, cuda_stream, &c));
   if (!xi || !v || !xi_bar || !v_bar || !theta_bar_dev) return GP_ERR_INVALID_ARG;
+  if (g->k > kMaxKGrad) return GP_ERR_UNSUPPORTED;
   return run_inverse_vjp(c, v, xi, xi_bar, v_bar, theta_bar_dev);
 }
 
@@ -238,6 +241,7 @@ gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_h
     return GP_ERR_INVALID_ARG;
   OpCtx c;
   GP_OK_OR_RETURN(make_ctx(g, kern, GP_OP_VJP, ws, ws_bytes, cuda_stream, &c));
+  if (g->k > kMaxKGrad) return GP_ERR_UNSUPPORTED;
   HostIO io;
   io.in_host[0] = xi_host;
   io.in_host[1] = v_host;

@@ -462,7 +462,8 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     float* rad2 = (float*)seg;                   // the segment ids of b1 are dead: reuse the buffer (tree order)
     if (k <= 16) knn_kernel<T, 16><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
     else if (k <= 32) knn_kernel<T, 32><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
-    else knn_kernel<T, 64><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
+    else if (k <= 64) knn_kernel<T, 64><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
+    else knn_kernel<T, 128><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
     GP_LAUNCH_CHECK();
   }
   GP_CUDA_OK(cudaEventRecord(E.ev[2], st));

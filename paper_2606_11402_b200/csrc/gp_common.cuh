@@ -10,7 +10,8 @@
 
 namespace gp {
 
-constexpr int kMaxK = 64;
+constexpr int kMaxK = 128;       // 64 < k <= 128: warp-per-point kernels (gp_large.cu), forward / inverse / logdet only
+constexpr int kMaxKGrad = 64;    // gradients, JVP, multi-sample calls
 constexpr int kMaxD = 4;
 constexpr int kCtrlBytes = 2048;
 constexpr int kAccSlots = 64;
@@ -302,5 +303,7 @@ gp_status run_geometry(const OpCtx& c, const void* xi, const void* v);
 gp_status run_jvp(const OpCtx& c, const void* xi, const void* v, const void* xi_dot, double sigma_dot, double ell_dot, void* v_dot);
 gp_status run_inverse_vjp(const OpCtx& c, const void* v, const void* xi, const void* xi_bar, void* v_bar, double* theta_bar);
 bool has_specialised(int dtype, int k, int d, int kind);
+// gp_large.cu: k > 64; op = GP_OP_FORWARD / INVERSE (in -> out) / LOGDET (logdet_dev)
+gp_status run_large(const OpCtx& c, int op, const void* in, void* out, double* logdet);
 
 }  // namespace gp

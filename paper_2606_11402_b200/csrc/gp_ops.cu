@@ -822,14 +822,17 @@ static gp_status logdet_t(const OpCtx& c, double* logdet, double* grad) {
 }
 
 gp_status run_forward(const OpCtx& c, const void* xi, void* v) {
+  if (c.g->k > kMaxKGrad) return run_large(c, GP_OP_FORWARD, xi, v, nullptr);
   return c.g->dtype == GP_F64 ? forward_t<double>(c, (const double*)xi, (double*)v)
                               : forward_t<float>(c, (const float*)xi, (float*)v);
 }
 gp_status run_inverse(const OpCtx& c, const void* v, void* xi) {
+  if (c.g->k > kMaxKGrad) return run_large(c, GP_OP_INVERSE, v, xi, nullptr);
   return c.g->dtype == GP_F64 ? inverse_t<double>(c, (const double*)v, (double*)xi)
                               : inverse_t<float>(c, (const float*)v, (float*)xi);
 }
 gp_status run_logdet(const OpCtx& c, double* logdet, double* grad) {
+  if (c.g->k > kMaxKGrad) return grad ? GP_ERR_UNSUPPORTED : run_large(c, GP_OP_LOGDET, nullptr, nullptr, logdet);
   return c.g->dtype == GP_F64 ? logdet_t<double>(c, logdet, grad) : logdet_t<float>(c, logdet, grad);
 }
 

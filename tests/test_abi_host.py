@@ -75,7 +75,7 @@ def test_argument_validation_is_synchronous_and_needs_no_gpu(gp):
     assert L.gp_forward(None, C.byref(kern), 1, 1, ws, big, None) == gp.GP_ERR_INVALID_ARG
     bad = gp.Kernel("se", 1.0, -0.1, 0.0).c()
     assert L.gp_forward(C.byref(g), C.byref(bad), 1, 1, ws, big, None) == gp.GP_ERR_INVALID_ARG
-    g2, _k2 = _graph(gp, k=80)
+    g2, _k2 = _graph(gp, k=200)
     assert L.gp_forward(C.byref(g2), C.byref(kern), 1, 1, ws, big, None) == gp.GP_ERR_UNSUPPORTED
     g3, _k3 = _graph(gp, n0=4)                                  # n0 < k
     assert L.gp_inverse(C.byref(g3), C.byref(kern), 1, 1, ws, big, None) == gp.GP_ERR_INVALID_ARG
