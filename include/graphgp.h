@@ -175,7 +175,7 @@ gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_h
  *   order   bit-reversed left-balanced k-d tree: node i at level l has children i+2^l, i+2^(l+1);
  *           split dimension = level mod d; ties by (coordinate, user id)             (R-3, R-4)
  *   kNN     k nearest among PRECEDING points in that order, ranked by (fp64 FMA-free squared distance,
- *           tree index)                                                                   (R-5)
+ *           tree index) (R-5); depth-first walk over the implicit tree restricted to indices < i
  *   depth   d_i = 1 + max_{j in c(i)} d_j by parallel fixed point; head depth 0
  *   sort    graph order = tree order stably sorted by depth; with GP_BUILD_SPATIAL_BATCHES points inside
  *           a batch are additionally ordered by Morton code of their coordinates (any order inside a batch is
@@ -187,7 +187,11 @@ gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_h
 enum { GP_BUILD_SPATIAL_BATCHES = 1,
        GP_BUILD_RADIUS_CLASSES = 2 /* inside a batch, order first by the class of the neighbourhood radius (distance to
                                       the farthest of the k neighbours, one class per two octaves), tight first, then
-                                      as GP_BUILD_SPATIAL_BATCHES says.  Optional and off by default. */ };
+                                      as GP_BUILD_SPATIAL_BATCHES says.  Optional and off by default. */,
+       GP_BUILD_PLAIN_KNN = 4      /* kNN by the plain walk (stack and candidate list in local memory) instead of the
+                                      shared-memory walk (stack + max-heap of the k best) used for d <= 3 and
+                                      k <= about 110.  Same result bit for bit; kept for comparison and as the path
+                                      for larger k or d.                                                        */ };
 gp_status gp_graph_build(const void* x_user, int64_t n, int32_t d, int32_t k, int64_t n0, int32_t dtype,
                          int32_t build_flags, int64_t* perm, void* x_graph, int32_t* nbr, int32_t* depth,
                          int64_t* batch_off_host, int32_t max_batches, int32_t* n_batches, void* ws,

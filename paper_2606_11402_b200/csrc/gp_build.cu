@@ -228,6 +228,123 @@ knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int64_t
   rad2[i] = (float)bd[k - 1];   // squared neighbourhood radius: orders the points inside a batch (sort_keys_kernel)
 }
 
+// ---- b2, fast form: the same walk on shared memory ---------------------------------------------------------------
+// Same walk as the plain kernel (pop, prune against the largest plane distance met on the way, visit, descend to the
+// near child, park the far child), restructured after its profile (N = 2^24, config 3: 358 GB of DRAM traffic from the
+// 830 bytes of local memory per thread): everything indexed at run time lives in SHARED memory, [slot][thread] so that
+// a warp's accesses never conflict whatever slots its lanes are at - the stack ({node, bound rounded DOWN to fp32},
+// at most one parked sibling per level) and the k best (d^2, index) pairs as a max-heap whose root is the current
+// k-th best, so accepting a candidate is one replace-root + sift-down (log2 k levels) instead of a rescan of all k.
+// Result identical to the plain kernel, bit for bit (tests/test_gpu_builder.py).  Measured and dropped (DESIGN.md
+// section 7): the stack-FREE traversal the paper points to (ref. Wald 2022b) with the list in registers,
+// lanes that fetch their next query themselves, and a vote that reconverges the warp every visit.
+constexpr int kKnnStack = 32;
+
+__device__ __forceinline__ bool key_gt(double da, int32_t ia, double db, int32_t ib) {
+  return da > db || (da == db && ia > ib);
+}
+
+// max-heap of k (d^2, index) keys at hd[slot * 128], hi[slot * 128]: put (nd, ni) at the root and sift it down
+__device__ __forceinline__ void heap_replace_root(double* hd, int32_t* hi, int k, double nd, int32_t ni) {
+  int pos = 0;
+  while (true) {
+    const int c1 = 2 * pos + 1;
+    if (c1 >= k) break;
+    int c = c1;
+    double dc = hd[c1 * 128];
+    int32_t ic = hi[c1 * 128];
+    if (c1 + 1 < k) {
+      const double d2 = hd[(c1 + 1) * 128];
+      const int32_t i2 = hi[(c1 + 1) * 128];
+      if (key_gt(d2, i2, dc, ic)) { c = c1 + 1; dc = d2; ic = i2; }
+    }
+    if (!key_gt(dc, ic, nd, ni)) break;
+    hd[pos * 128] = dc;
+    hi[pos * 128] = ic;
+    pos = c;
+  }
+  hd[pos * 128] = nd;
+  hi[pos * 128] = ni;
+}
+
+template <typename T, int D>
+__global__ void __launch_bounds__(128)
+knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_threads, int32_t* __restrict__ nbr,
+              float* __restrict__ rad2) {
+  extern __shared__ double knn_smem[];
+  double* hd = knn_smem + threadIdx.x;                                   // [k][128]
+  int2* stk = reinterpret_cast<int2*>(knn_smem + (size_t)k * 128) + threadIdx.x;   // [kKnnStack][128]
+  int32_t* hi = reinterpret_cast<int32_t*>(knn_smem + (size_t)(k + kKnnStack) * 128) + threadIdx.x;   // [k][128]
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n_threads) return;
+  // thread t -> level l, heap position q -> bit-reversed position p -> tree index i: the queries of one warp are
+  // consecutive leaves of the same level, i.e. spatial neighbours
+  const int l = 63 - __clzll((unsigned long long)(t + 1));
+  const int64_t q = t - (((int64_t)1 << l) - 1);
+  const int64_t p = l == 0 ? 0 : (int64_t)(__brevll((unsigned long long)q) >> (64 - l));
+  const int64_t i = (((int64_t)1 << l) - 1) + p;
+  if (i >= n || i < n0) return;
+
+  const double inf = __longlong_as_double(0x7ff0000000000000LL);
+  double xi[D];
+#pragma unroll
+  for (int a = 0; a < D; ++a) xi[a] = (double)x[i * D + a];
+  for (int a = 0; a < k; ++a) { hd[a * 128] = inf; hi[a * 128] = 0x7fffffff; }   // k sentinels: no separate fill phase
+  double wd = inf;                             // root of the heap: the k-th best so far
+  int32_t wi = 0x7fffffff;
+  const uint32_t lim = (uint32_t)i;            // nodes < lim exist for this query (preceding points only)
+  int sp = 0;
+  int32_t curr = 0;
+  float bound = 0.0f;                          // lower bound of d^2 for everything below curr
+  bool have = true;
+  while (true) {
+    if (!have) {
+      if (sp == 0) break;
+      const int2 e = stk[--sp * 128];
+      curr = e.x;
+      bound = __int_as_float(e.y);
+      have = true;
+    }
+    if ((double)bound > wd) { have = false; continue; }
+    const T* xc = x + (int64_t)curr * D;
+    const int lc = 31 - __clz(curr + 1);
+    const int dim = lc % D;
+    double acc = 0.0, diff = 0.0;
+#pragma unroll
+    for (int a = 0; a < D; ++a) {
+      const double dx = __dsub_rn(xi[a], (double)__ldg(xc + a));
+      const double sq = __dmul_rn(dx, dx);
+      acc = a == 0 ? sq : __dadd_rn(acc, sq);
+      diff = a == dim ? dx : diff;
+    }
+    if (key_gt(wd, wi, acc, curr)) {
+      heap_replace_root(hd, hi, k, acc, curr);
+      wd = hd[0];
+      wi = hi[0];
+    }
+    const uint32_t half = 1u << lc, room = lim - (uint32_t)curr;   // a child curr + s exists iff s < room
+    const bool near_left = diff < 0.0;
+    const uint32_t near_s = near_left ? half : 2u * half, far_s = near_left ? 2u * half : half;
+    if (far_s < room) {
+      const float fb = fmaxf(__double2float_rd(__dmul_rn(diff, diff)), bound);
+      if (!((double)fb > wd)) stk[sp++ * 128] = make_int2(curr + (int32_t)far_s, __float_as_int(fb));
+    }
+    if (near_s < room) curr += (int32_t)near_s;
+    else have = false;
+  }
+  // nearest first: pop the heap from the back
+  int32_t* out = nbr + (i - n0) * k;
+  rad2[i] = (float)wd;     // squared neighbourhood radius: orders the points inside a batch (sort_keys_kernel)
+  for (int m = k - 1; m >= 0; --m) {
+    out[m] = hi[0];
+    if (m > 0) {
+      const double ld = hd[m * 128];
+      const int32_t li = hi[m * 128];
+      heap_replace_root(hd, hi, m, ld, li);
+    }
+  }
+}
+
 // ---- b3: depth ----------------------------------------------------------------------------------------
 __global__ void max_depth_kernel(const int32_t* __restrict__ depth, int64_t n, unsigned long long* out) {
   int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -460,7 +577,16 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     int64_t n_threads = ((int64_t)2 << shape.lam) - 1;
     unsigned long long* ovf = &ctrl->n_bad;      // zeroed above; read back with the depth watchdog below
     float* rad2 = (float*)seg;                   // the segment ids of b1 are dead: reuse the buffer (tree order)
-    if (k <= 16) knn_kernel<T, 16><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
+    const bool plain = (flags & GP_BUILD_PLAIN_KNN) != 0;
+    const size_t sm_bytes = (size_t)128 * (12 * (size_t)k + 8 * kKnnStack);
+    if (!plain && d <= 3 && sm_bytes <= 200 * 1024) {
+#define GP_KNN_SM(DD) { \
+      GP_CUDA_OK(cudaFuncSetAttribute(knn_sm_kernel<T, DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); \
+      knn_sm_kernel<T, DD><<<nblk(n_threads, 128), 128, sm_bytes, st>>>(x_tree, n, n0, k, n_threads, nbr_tree, rad2); }
+      if (d == 1) GP_KNN_SM(1) else if (d == 2) GP_KNN_SM(2) else GP_KNN_SM(3)
+#undef GP_KNN_SM
+    }
+    else if (k <= 16) knn_kernel<T, 16><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
     else if (k <= 32) knn_kernel<T, 32><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
     else if (k <= 64) knn_kernel<T, 64><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
     else knn_kernel<T, 128><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);

@@ -111,3 +111,22 @@ def test_builder_large_sampled_rows(gp, orc):
     assert G.batch_off[0] == n0 and G.batch_off[-1] == n
     assert np.array_equal(np.flatnonzero(np.diff(depth[n0:])) + n0 + 1, G.batch_off[1:-1])
     assert (np.sort(nbr, axis=1)[:, 1:] != np.sort(nbr, axis=1)[:, :-1]).all()
+
+
+@pytest.mark.parametrize("n,d,k,dtype", [(20000, 3, 16, "f32"), (20000, 2, 32, "f32"), (9000, 1, 5, "f64"),
+                                         (12000, 3, 64, "f32"), (7000, 2, 3, "f64"), (30000, 3, 100, "f32")])
+def test_builder_knn_paths_agree_row_for_row(gp, orc, n, d, k, dtype):
+    """The shared-memory kNN walk (default) and the plain one (GP_BUILD_PLAIN_KNN) give the same rows in the same
+    (nearest first, ties by tree index) order, and that order is the oracle's."""
+    rng = np.random.default_rng(1000 + k)
+    x = rng.standard_normal((n, d)).astype(np.float32 if dtype == "f32" else np.float64)
+    x[50:90] = x[10:50]                                       # exact duplicates: ties in d^2
+    n0 = 128
+    fast = build_gpu(gp, x, k, n0, 0)
+    plain = build_gpu(gp, x, k, n0, gp.GP_BUILD_PLAIN_KNN)
+    assert np.array_equal(fast.perm.cpu().numpy(), plain.perm.cpu().numpy())
+    assert np.array_equal(fast.nbr.cpu().numpy(), plain.nbr.cpu().numpy())
+    assert np.array_equal(fast.depth.cpu().numpy(), plain.depth.cpu().numpy())
+    if k <= 64:
+        ref = orc.build_graph(x.astype(np.float64), k, n0)
+        assert np.array_equal(fast.nbr.cpu().numpy(), ref.nbr)
