@@ -190,7 +190,7 @@ enum { GP_BUILD_SPATIAL_BATCHES = 1,
                                       as GP_BUILD_SPATIAL_BATCHES says.  Optional and off by default. */,
        GP_BUILD_PLAIN_KNN = 4      /* kNN by the plain walk (stack and candidate list in local memory) instead of the
                                       shared-memory walk (stack + max-heap of the k best) used for d <= 3 and
-                                      k <= about 110.  Same result bit for bit; kept for comparison and as the path
+                                      every k <= 128.  Same result bit for bit; kept for comparison and as the path
                                       for larger k or d.                                                        */ };
 gp_status gp_graph_build(const void* x_user, int64_t n, int32_t d, int32_t k, int64_t n0, int32_t dtype,
                          int32_t build_flags, int64_t* perm, void* x_graph, int32_t* nbr, int32_t* depth,

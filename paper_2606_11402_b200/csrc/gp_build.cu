@@ -239,42 +239,46 @@ knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int64_t
 // section 7): the stack-FREE traversal the paper points to (ref. Wald 2022b) with the list in registers,
 // lanes that fetch their next query themselves, and a vote that reconverges the warp every visit.
 constexpr int kKnnStack = 32;
+// One warp per CTA: a CTA gives its shared memory back when its slowest warp is done, and the queries of different
+// warps differ 2-3x in length on clustered inputs (measured at N = 2^24, kNN stage, CTAs of 128 / 64 / 32 threads:
+// config 3 113 / 102 / 79 ms, config 4 81 / 66 / 64 ms).
+constexpr int kKnnThreads = 32;
 
 __device__ __forceinline__ bool key_gt(double da, int32_t ia, double db, int32_t ib) {
   return da > db || (da == db && ia > ib);
 }
 
-// max-heap of k (d^2, index) keys at hd[slot * 128], hi[slot * 128]: put (nd, ni) at the root and sift it down
+// max-heap of k (d^2, index) keys at hd[slot * kKnnThreads], hi[slot * kKnnThreads]: put (nd, ni) at the root and sift it down
 __device__ __forceinline__ void heap_replace_root(double* hd, int32_t* hi, int k, double nd, int32_t ni) {
   int pos = 0;
   while (true) {
     const int c1 = 2 * pos + 1;
     if (c1 >= k) break;
     int c = c1;
-    double dc = hd[c1 * 128];
-    int32_t ic = hi[c1 * 128];
+    double dc = hd[c1 * kKnnThreads];
+    int32_t ic = hi[c1 * kKnnThreads];
     if (c1 + 1 < k) {
-      const double d2 = hd[(c1 + 1) * 128];
-      const int32_t i2 = hi[(c1 + 1) * 128];
+      const double d2 = hd[(c1 + 1) * kKnnThreads];
+      const int32_t i2 = hi[(c1 + 1) * kKnnThreads];
       if (key_gt(d2, i2, dc, ic)) { c = c1 + 1; dc = d2; ic = i2; }
     }
     if (!key_gt(dc, ic, nd, ni)) break;
-    hd[pos * 128] = dc;
-    hi[pos * 128] = ic;
+    hd[pos * kKnnThreads] = dc;
+    hi[pos * kKnnThreads] = ic;
     pos = c;
   }
-  hd[pos * 128] = nd;
-  hi[pos * 128] = ni;
+  hd[pos * kKnnThreads] = nd;
+  hi[pos * kKnnThreads] = ni;
 }
 
 template <typename T, int D>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kKnnThreads)
 knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_threads, int32_t* __restrict__ nbr,
               float* __restrict__ rad2) {
   extern __shared__ double knn_smem[];
-  double* hd = knn_smem + threadIdx.x;                                   // [k][128]
-  int2* stk = reinterpret_cast<int2*>(knn_smem + (size_t)k * 128) + threadIdx.x;   // [kKnnStack][128]
-  int32_t* hi = reinterpret_cast<int32_t*>(knn_smem + (size_t)(k + kKnnStack) * 128) + threadIdx.x;   // [k][128]
+  double* hd = knn_smem + threadIdx.x;                                   // [k][kKnnThreads]
+  int2* stk = reinterpret_cast<int2*>(knn_smem + (size_t)k * kKnnThreads) + threadIdx.x;   // [kKnnStack][kKnnThreads]
+  int32_t* hi = reinterpret_cast<int32_t*>(knn_smem + (size_t)(k + kKnnStack) * kKnnThreads) + threadIdx.x;   // [k][kKnnThreads]
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n_threads) return;
   // thread t -> level l, heap position q -> bit-reversed position p -> tree index i: the queries of one warp are
@@ -289,7 +293,7 @@ knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_t
   double xi[D];
 #pragma unroll
   for (int a = 0; a < D; ++a) xi[a] = (double)x[i * D + a];
-  for (int a = 0; a < k; ++a) { hd[a * 128] = inf; hi[a * 128] = 0x7fffffff; }   // k sentinels: no separate fill phase
+  for (int a = 0; a < k; ++a) { hd[a * kKnnThreads] = inf; hi[a * kKnnThreads] = 0x7fffffff; }   // k sentinels: no separate fill phase
   double wd = inf;                             // root of the heap: the k-th best so far
   int32_t wi = 0x7fffffff;
   const uint32_t lim = (uint32_t)i;            // nodes < lim exist for this query (preceding points only)
@@ -300,7 +304,7 @@ knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_t
   while (true) {
     if (!have) {
       if (sp == 0) break;
-      const int2 e = stk[--sp * 128];
+      const int2 e = stk[--sp * kKnnThreads];
       curr = e.x;
       bound = __int_as_float(e.y);
       have = true;
@@ -327,7 +331,7 @@ knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_t
     const uint32_t near_s = near_left ? half : 2u * half, far_s = near_left ? 2u * half : half;
     if (far_s < room) {
       const float fb = fmaxf(__double2float_rd(__dmul_rn(diff, diff)), bound);
-      if (!((double)fb > wd)) stk[sp++ * 128] = make_int2(curr + (int32_t)far_s, __float_as_int(fb));
+      if (!((double)fb > wd)) stk[sp++ * kKnnThreads] = make_int2(curr + (int32_t)far_s, __float_as_int(fb));
     }
     if (near_s < room) curr += (int32_t)near_s;
     else have = false;
@@ -338,8 +342,8 @@ knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_t
   for (int m = k - 1; m >= 0; --m) {
     out[m] = hi[0];
     if (m > 0) {
-      const double ld = hd[m * 128];
-      const int32_t li = hi[m * 128];
+      const double ld = hd[m * kKnnThreads];
+      const int32_t li = hi[m * kKnnThreads];
       heap_replace_root(hd, hi, m, ld, li);
     }
   }
@@ -597,11 +601,11 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     unsigned long long* ovf = &ctrl->n_bad;      // zeroed above; read back with the depth watchdog below
     float* rad2 = (float*)seg;                   // the segment ids of b1 are dead: reuse the buffer (tree order)
     const bool plain = (flags & GP_BUILD_PLAIN_KNN) != 0;
-    const size_t sm_bytes = (size_t)128 * (12 * (size_t)k + 8 * kKnnStack);
+    const size_t sm_bytes = (size_t)kKnnThreads * (12 * (size_t)k + 8 * kKnnStack);
     if (!plain && d <= 3 && sm_bytes <= 200 * 1024) {
 #define GP_KNN_SM(DD) { \
       GP_CUDA_OK(cudaFuncSetAttribute(knn_sm_kernel<T, DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); \
-      knn_sm_kernel<T, DD><<<nblk(n_threads, 128), 128, sm_bytes, st>>>(x_tree, n, n0, k, n_threads, nbr_tree, rad2); }
+      knn_sm_kernel<T, DD><<<nblk(n_threads, kKnnThreads), kKnnThreads, sm_bytes, st>>>(x_tree, n, n0, k, n_threads, nbr_tree, rad2); }
       if (d == 1) GP_KNN_SM(1) else if (d == 2) GP_KNN_SM(2) else GP_KNN_SM(3)
 #undef GP_KNN_SM
     }
