@@ -45,7 +45,9 @@ typedef enum {
                              logdet and the builder; k <= 64 for the gradient, JVP and multi-sample calls */
   GP_ERR_NOT_PD = 3,
   GP_ERR_CUDA = 4,
-  GP_ERR_WORKSPACE = 5 /* ws == NULL or ws_bytes < gp_workspace_bytes() */
+  GP_ERR_WORKSPACE = 5, /* ws == NULL or ws_bytes < gp_workspace_bytes() */
+  GP_ERR_TOO_LARGE = 6  /* gp_logdet_noalloc only: n0 > GP_NOALLOC_MAX_N0 or k > GP_NOALLOC_MAX_K (its scratch is a
+                           fixed device array); use gp_logdet with a workspace instead */
 } gp_status;
 
 typedef enum { GP_KERNEL_SE = 0, GP_KERNEL_MATERN32 = 1, GP_KERNEL_EXP = 2 } gp_kernel_kind;
@@ -111,6 +113,25 @@ gp_status gp_inverse(const gp_graph* g, const gp_kernel* kern, const void* v, vo
  * larger gp_workspace_bytes(g, GP_OP_VJP) (the head carries 2 n0 extra rows), else GP_ERR_WORKSPACE.         */
 gp_status gp_logdet(const gp_graph* g, const gp_kernel* kern, double* logdet_dev, double* dlogdet_dtheta_dev,
                     void* ws, size_t ws_bytes, void* cuda_stream);
+
+/* gp_logdet for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): no workspace argument.  Same quantity as gp_logdet (Eq. 2 for
+ * s_i^2), without the gradient.  The scratch - the n0 x n0 fp64 matrix of the dense head (Alg. 1 line 1) and the
+ * accumulators - is ONE fixed array in device memory inside the library, gp_logdet_noalloc_scratch_bytes() = 8 MiB +
+ * 4 KiB, which every GPU that loads the library holds until the process exits.  Hence the limits: n0 <=
+ * GP_NOALLOC_MAX_N0 and k <= GP_NOALLOC_MAX_K, any n; beyond them the call returns GP_ERR_TOO_LARGE and launches
+ * nothing.  The call enqueues kernels and one memset on `cuda_stream` and calls no cudaMalloc / cudaFree, creates no
+ * stream or event, and uses no allocating library routine.  fp64 arithmetic whatever g->dtype; shared-memory kernels,
+ * roughly an order of magnitude slower than gp_logdet.
+ * g, kern: as for gp_logdet (g->batch_off is not used beyond validation).  logdet_dev: device double[1] (out), NaN if
+ * any conditional or head pivot was not positive (there is no workspace to query with gp_check_errors).
+ * ALL calls share the one array, and it keeps the last call's contents (what must start at zero is cleared by every
+ * call): two calls whose GPU work overlaps - different streams, or host threads - on the same device RACE; callers
+ * serialise them.  Per-device state: the array's device address, taken once per device on first use.             */
+#define GP_NOALLOC_MAX_N0 1024
+#define GP_NOALLOC_MAX_K 64
+gp_status gp_logdet_noalloc(const gp_graph* g, const gp_kernel* kern, double* logdet_dev, void* cuda_stream);
+size_t gp_logdet_noalloc_scratch_bytes(void);
 
 /* Vector-Jacobian product of gp_forward ("backward derivatives"): given xi, v = forward(xi)
  * and a cotangent v_bar, returns xi_bar [n] and theta_bar = (d/dsigma, d/dell) of <v_bar, forward(xi; theta)>.

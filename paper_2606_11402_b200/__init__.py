@@ -16,7 +16,7 @@ import numpy as np
 
 from .build import LIB, build_library
 
-GP_OK, GP_ERR_INVALID_ARG, GP_ERR_UNSUPPORTED, GP_ERR_NOT_PD, GP_ERR_CUDA, GP_ERR_WORKSPACE = range(6)
+GP_OK, GP_ERR_INVALID_ARG, GP_ERR_UNSUPPORTED, GP_ERR_NOT_PD, GP_ERR_CUDA, GP_ERR_WORKSPACE, GP_ERR_TOO_LARGE = range(7)
 GP_F32, GP_F64 = 0, 1
 GP_OP_FORWARD, GP_OP_INVERSE, GP_OP_LOGDET, GP_OP_VJP, GP_OP_BUILD, GP_OP_FORWARD_MULTI, GP_OP_INVERSE_MULTI = range(7)
 GP_FLAG_PER_BATCH_LAUNCH, GP_FLAG_GENERIC_KERNEL, GP_FLAG_FLOW_CARRY, GP_FLAG_FLOW_WEIGHTS = 1, 2, 4, 8
@@ -26,7 +26,8 @@ KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
 EXPORTS = ["gp_workspace_bytes", "gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host",
            "gp_inverse_host", "gp_logdet_host", "gp_vjp_host", "gp_graph_build", "gp_graph_build_workspace_bytes", "gp_graph_build_times",
            "gp_check_errors", "gp_status_string", "gp_has_specialised", "gp_launch_count", "gp_kernel_time_enable",
-           "gp_kernel_time_last", "gp_measure_alu_peak", "gp_workspace_bytes_multi", "gp_forward_multi", "gp_inverse_multi", "gp_jvp", "gp_inverse_vjp"]
+           "gp_kernel_time_last", "gp_measure_alu_peak", "gp_workspace_bytes_multi", "gp_forward_multi", "gp_inverse_multi", "gp_jvp", "gp_inverse_vjp",
+           "gp_logdet_noalloc", "gp_logdet_noalloc_scratch_bytes"]
 
 
 class GraphGPError(RuntimeError):
@@ -94,6 +95,10 @@ def lib():
         L.gp_forward_multi.restype = C.c_int
         L.gp_inverse_multi.restype = C.c_int
         L.gp_measure_alu_peak.argtypes = [vp, C.c_int32, vp, sz, vp]
+        L.gp_logdet_noalloc.argtypes = gk + [vp, vp]
+        L.gp_logdet_noalloc_scratch_bytes.argtypes = []
+        L.gp_logdet_noalloc_scratch_bytes.restype = C.c_size_t
+        L.gp_logdet_noalloc.restype = C.c_int
         L.gp_measure_alu_peak.restype = C.c_int
         for name in ("gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host", "gp_inverse_host",
                      "gp_vjp_host", "gp_logdet_host", "gp_graph_build", "gp_graph_build_times", "gp_check_errors"):
@@ -308,6 +313,21 @@ def gp_logdet(graph: Graph, kern: Kernel, grad: bool = False, stream=None):
     _check(lib().gp_logdet(C.byref(g), C.byref(k), out.data_ptr(), gout.data_ptr() if grad else None,
                            ws.data_ptr(), ws.numel(), _stream_ptr(stream)), "gp_logdet")
     return (out, gout) if grad else out
+
+
+def gp_logdet_noalloc(graph: Graph, kern: Kernel, out, stream=None):
+    """gp_logdet without a workspace (fixed scratch array inside the library; n0 <= 1024, k <= 64, else GraphGPError with
+    GP_ERR_TOO_LARGE).  out: caller's device float64[1].  Calls that overlap on the GPU race on the scratch."""
+    torch = _torch()
+    if not isinstance(out, torch.Tensor) or out.dtype != torch.float64 or out.numel() < 1 or out.device != graph.x.device:
+        raise TypeError("gp_logdet_noalloc: out must be a float64 tensor with >= 1 element on the graph's device")
+    g, k = graph.c(), kern.c()
+    _check(lib().gp_logdet_noalloc(C.byref(g), C.byref(k), out.data_ptr(), _stream_ptr(stream)), "gp_logdet_noalloc")
+    return out
+
+
+def logdet_noalloc_scratch_bytes() -> int:
+    return int(lib().gp_logdet_noalloc_scratch_bytes())
 
 
 def gp_vjp(graph: Graph, kern: Kernel, xi, v, v_bar, stream=None):

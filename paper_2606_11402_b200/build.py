@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgraphgp.so")
-SOURCES = ["gp_api.cu", "gp_ops.cu", "gp_head.cu", "gp_vjp.cu", "gp_build.cu", "gp_peak.cu", "gp_multi.cu", "gp_jvp.cu", "gp_large.cu"]
+SOURCES = ["gp_api.cu", "gp_ops.cu", "gp_head.cu", "gp_vjp.cu", "gp_build.cu", "gp_peak.cu", "gp_multi.cu", "gp_jvp.cu", "gp_large.cu", "gp_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
 

@@ -271,6 +271,7 @@ const char* gp_status_string(gp_status s) {
     case GP_ERR_NOT_PD: return "a conditional covariance was not positive definite";
     case GP_ERR_CUDA: return "CUDA error or no CUDA device";
     case GP_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case GP_ERR_TOO_LARGE: return "size beyond the fixed scratch of gp_logdet_noalloc (n0 <= 1024, k <= 64): use gp_logdet";
   }
   return "unknown status";
 }
