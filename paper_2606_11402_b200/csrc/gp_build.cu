@@ -238,7 +238,6 @@ knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int64_t
 // Result identical to the plain kernel, bit for bit (tests/test_gpu_builder.py).  Measured and dropped (DESIGN.md
 // section 7): the stack-FREE traversal the paper points to (ref. Wald 2022b) with the list in registers,
 // lanes that fetch their next query themselves, and a vote that reconverges the warp every visit.
-constexpr int kKnnStack = 32;
 // One warp per CTA: a CTA gives its shared memory back when its slowest warp is done, and the queries of different
 // warps differ 2-3x in length on clustered inputs (measured at N = 2^24, kNN stage, CTAs of 128 / 64 / 32 threads:
 // config 3 113 / 102 / 79 ms, config 4 81 / 66 / 64 ms).
@@ -273,12 +272,12 @@ __device__ __forceinline__ void heap_replace_root(double* hd, int32_t* hi, int k
 
 template <typename T, int D>
 __global__ void __launch_bounds__(kKnnThreads)
-knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_threads, int32_t* __restrict__ nbr,
-              float* __restrict__ rad2) {
+knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int nlev, int64_t n_threads,
+              int32_t* __restrict__ nbr, float* __restrict__ rad2) {
   extern __shared__ double knn_smem[];
-  double* hd = knn_smem + threadIdx.x;                                   // [k][kKnnThreads]
-  int2* stk = reinterpret_cast<int2*>(knn_smem + (size_t)k * kKnnThreads) + threadIdx.x;   // [kKnnStack][kKnnThreads]
-  int32_t* hi = reinterpret_cast<int32_t*>(knn_smem + (size_t)(k + kKnnStack) * kKnnThreads) + threadIdx.x;   // [k][kKnnThreads]
+  double* hd = knn_smem + threadIdx.x;                                                           // [k][kKnnThreads]
+  int32_t* hi = reinterpret_cast<int32_t*>(knn_smem + (size_t)k * kKnnThreads) + threadIdx.x;     // [k][kKnnThreads]
+  float* bnd = reinterpret_cast<float*>(hi - threadIdx.x + (size_t)k * kKnnThreads) + threadIdx.x;   // [nlev][kKnnThreads]
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= n_threads) return;
   // thread t -> level l, heap position q -> bit-reversed position p -> tree index i: the queries of one warp are
@@ -297,21 +296,29 @@ knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_t
   double wd = inf;                             // root of the heap: the k-th best so far
   int32_t wi = 0x7fffffff;
   const uint32_t lim = (uint32_t)i;            // nodes < lim exist for this query (preceding points only)
-  int sp = 0;
+  // The "stack": at most one parked sibling per level, and WHICH node it is follows from the path - node (level l,
+  // position p) has children (l + 1, p) and (l + 1, p + 2^l), so bit t of p is the turn taken at level t and the
+  // sibling parked at level L is (L, (p mod 2^(L-1)) + (1 - bit_{L-1}(p)) 2^(L-1)).  So only the BOUND of a parked
+  // sibling is stored (fp32, [level][thread]) and a bit mask says which levels hold one: 4 bytes per level instead of
+  // 8 per entry, which is what limits the warps per SM.  The deepest parked level is the top of the stack.
+  uint32_t parked = 0;
   int32_t curr = 0;
+  int lc = 0;                                  // level of curr
   float bound = 0.0f;                          // lower bound of d^2 for everything below curr
   bool have = true;
   while (true) {
     if (!have) {
-      if (sp == 0) break;
-      const int2 e = stk[--sp * kKnnThreads];
-      curr = e.x;
-      bound = __int_as_float(e.y);
+      if (!parked) break;
+      const int L = 31 - __clz(parked);
+      parked &= ~(1u << L);
+      const uint32_t p = (uint32_t)curr + 1u - (1u << lc), hb = 1u << (L - 1);
+      curr = (int32_t)((2u * hb - 1u) + (p & (hb - 1u)) + ((p & hb) ^ hb));
+      lc = L;
+      bound = bnd[L * kKnnThreads];
       have = true;
     }
     if ((double)bound > wd) { have = false; continue; }
     const T* xc = x + (int64_t)curr * D;
-    const int lc = 31 - __clz(curr + 1);
     const int dim = lc % D;
     double acc = 0.0, diff = 0.0;
 #pragma unroll
@@ -329,12 +336,19 @@ knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int64_t n_t
     const uint32_t half = 1u << lc, room = lim - (uint32_t)curr;   // a child curr + s exists iff s < room
     const bool near_left = diff < 0.0;
     const uint32_t near_s = near_left ? half : 2u * half, far_s = near_left ? 2u * half : half;
-    if (far_s < room) {
-      const float fb = fmaxf(__double2float_rd(__dmul_rn(diff, diff)), bound);
-      if (!((double)fb > wd)) stk[sp++ * kKnnThreads] = make_int2(curr + (int32_t)far_s, __float_as_int(fb));
+    const float fb = fmaxf(__double2float_rd(__dmul_rn(diff, diff)), bound);
+    const bool far_go = far_s < room && !((double)fb > wd);
+    if (near_s < room) {
+      if (far_go) { bnd[(lc + 1) * kKnnThreads] = fb; parked |= 2u << lc; }
+      curr += (int32_t)near_s;
+      ++lc;
+    } else if (far_go) {                         // only the far child exists (it has the smaller index): no turn to remember
+      curr += (int32_t)far_s;
+      ++lc;
+      bound = fb;
+    } else {
+      have = false;
     }
-    if (near_s < room) curr += (int32_t)near_s;
-    else have = false;
   }
   // nearest first: pop the heap from the back
   int32_t* out = nbr + (i - n0) * k;
@@ -601,11 +615,12 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     unsigned long long* ovf = &ctrl->n_bad;      // zeroed above; read back with the depth watchdog below
     float* rad2 = (float*)seg;                   // the segment ids of b1 are dead: reuse the buffer (tree order)
     const bool plain = (flags & GP_BUILD_PLAIN_KNN) != 0;
-    const size_t sm_bytes = (size_t)kKnnThreads * (12 * (size_t)k + 8 * kKnnStack);
+    const int nlev = shape.lam + 2;                // levels 0 .. lam + 1 can be indexed (level 0 is never parked)
+    const size_t sm_bytes = (size_t)kKnnThreads * (12 * (size_t)k + 4 * (size_t)nlev);
     if (!plain && d <= 3 && sm_bytes <= 200 * 1024) {
 #define GP_KNN_SM(DD) { \
       GP_CUDA_OK(cudaFuncSetAttribute(knn_sm_kernel<T, DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); \
-      knn_sm_kernel<T, DD><<<nblk(n_threads, kKnnThreads), kKnnThreads, sm_bytes, st>>>(x_tree, n, n0, k, n_threads, nbr_tree, rad2); }
+      knn_sm_kernel<T, DD><<<nblk(n_threads, kKnnThreads), kKnnThreads, sm_bytes, st>>>(x_tree, n, n0, k, nlev, n_threads, nbr_tree, rad2); }
       if (d == 1) GP_KNN_SM(1) else if (d == 2) GP_KNN_SM(2) else GP_KNN_SM(3)
 #undef GP_KNN_SM
     }
