@@ -248,7 +248,7 @@ def run_graft(args):
     x_user = torch.as_tensor(x_h, device=dev)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
-    G = gp.gp_graph_build(x_user, cfg.k, cfg.n0)
+    G = gp.gp_graph_build(x_user, cfg.k, cfg.n0, gp.GP_BUILD_SPATIAL_BATCHES | (gp.GP_BUILD_PLAIN_KNN if args.plain_knn else 0))
     torch.cuda.synchronize()
     build_wall = time.perf_counter() - t0
     del x_user
@@ -547,6 +547,8 @@ def main():
     ap.add_argument("--multi", type=int, default=0, help="also time gp_forward_multi / gp_inverse_multi with this many "
                                                          "samples per call (reported under \"multi\")")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--plain-knn", action="store_true", help="build the graph with the plain (local-memory) kNN walk, "
+                    "GP_BUILD_PLAIN_KNN; same graph bit for bit, for builder comparisons")
     ap.add_argument("--cpu-seconds", type=float, default=30.0, help="target CPU time of the cpu_baseline sample")
     ap.add_argument("--reference-points", type=int, default=1 << 16)
     args = ap.parse_args()
