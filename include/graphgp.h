@@ -194,7 +194,8 @@ gp_status gp_vjp_host(const gp_graph* g, const gp_kernel* kern, const void* xi_h
 
 /* Graph construction, separately timed, "plain":
  *   order   bit-reversed left-balanced k-d tree: node i at level l has children i+2^l, i+2^(l+1);
- *           split dimension = level mod d; ties by (coordinate, user id)             (R-3, R-4)
+ *           split dimension = level mod d; ties by (coordinate, user id)             (R-3, R-4);
+ *           sort-based: one radix sort per dimension, then a stable split of the sorted lists per level
  *   kNN     k nearest among PRECEDING points in that order, ranked by (fp64 FMA-free squared distance,
  *           tree index) (R-5); depth-first walk over the implicit tree restricted to indices < i
  *   depth   d_i = 1 + max_{j in c(i)} d_j by parallel fixed point; head depth 0
@@ -212,7 +213,10 @@ enum { GP_BUILD_SPATIAL_BATCHES = 1,
        GP_BUILD_PLAIN_KNN = 4      /* kNN by the plain walk (stack and candidate list in local memory) instead of the
                                       shared-memory walk (stack + max-heap of the k best) used for d <= 3 and
                                       every k <= 128.  Same result bit for bit; kept for comparison and as the path
-                                      for larger k or d.                                                        */ };
+                                      for larger k or d.                                                        */,
+       GP_BUILD_PLAIN_ORDER = 8    /* tree order by one radix sort of (subtree, coordinate rank) keys per level
+                                      instead of the presorted per-dimension lists split stably per level (one
+                                      sort per dimension in all).  Same order bit for bit; kept for comparison. */ };
 gp_status gp_graph_build(const void* x_user, int64_t n, int32_t d, int32_t k, int64_t n0, int32_t dtype,
                          int32_t build_flags, int64_t* perm, void* x_graph, int32_t* nbr, int32_t* depth,
                          int64_t* batch_off_host, int32_t max_batches, int32_t* n_batches, void* ws,

@@ -20,7 +20,7 @@ GP_OK, GP_ERR_INVALID_ARG, GP_ERR_UNSUPPORTED, GP_ERR_NOT_PD, GP_ERR_CUDA, GP_ER
 GP_F32, GP_F64 = 0, 1
 GP_OP_FORWARD, GP_OP_INVERSE, GP_OP_LOGDET, GP_OP_VJP, GP_OP_BUILD, GP_OP_FORWARD_MULTI, GP_OP_INVERSE_MULTI = range(7)
 GP_FLAG_PER_BATCH_LAUNCH, GP_FLAG_GENERIC_KERNEL, GP_FLAG_FLOW_CARRY, GP_FLAG_FLOW_WEIGHTS = 1, 2, 4, 8
-GP_BUILD_SPATIAL_BATCHES, GP_BUILD_RADIUS_CLASSES, GP_BUILD_PLAIN_KNN = 1, 2, 4
+GP_BUILD_SPATIAL_BATCHES, GP_BUILD_RADIUS_CLASSES, GP_BUILD_PLAIN_KNN, GP_BUILD_PLAIN_ORDER = 1, 2, 4, 8
 KIND_ID = {"se": 0, "matern32": 1, "exp": 2}
 
 EXPORTS = ["gp_workspace_bytes", "gp_forward", "gp_inverse", "gp_logdet", "gp_vjp", "gp_forward_host",

@@ -14,6 +14,7 @@
 //
 // Sorting and scanning use CUB (a library primitive on a path that is not the hot path).
 #include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_partition.cuh>
 
 #include "gp_common.cuh"
 
@@ -102,7 +103,7 @@ __host__ __device__ inline TreeShape tree_shape(int64_t n) {
 // nodes of the last level lying in the subtree rooted at (l, p): positions q < mlast with q mod 2^l == p
 __host__ __device__ inline int64_t last_level_in(const TreeShape& s, int l, int64_t p) {
   int64_t step = (int64_t)1 << l;
-  return p < s.mlast ? (s.mlast - p + step - 1) / step : 0;
+  return p < s.mlast ? (s.mlast - p + step - 1) >> l : 0;       // step is a power of two: shifts, not divisions
 }
 __host__ __device__ inline int64_t subtree_size(const TreeShape& s, int l, int64_t p) {
   if (l > s.lam) return 0;
@@ -112,7 +113,8 @@ __host__ __device__ inline int64_t subtree_size(const TreeShape& s, int l, int64
 // elements in subtrees (l, 0..p-1)
 __host__ __device__ inline int64_t subtree_prefix(const TreeShape& s, int l, int64_t p) {
   int64_t step = (int64_t)1 << l;
-  int64_t last = (s.mlast / step) * p + (s.mlast % step < p ? s.mlast % step : p);
+  int64_t rem = s.mlast & (step - 1);
+  int64_t last = (s.mlast >> l) * p + (rem < p ? rem : p);
   if (l == s.lam) return last;
   return p * (((int64_t)1 << (s.lam - l)) - 1) + last;
 }
@@ -133,6 +135,53 @@ __global__ void level_split_kernel(const uint64_t* __restrict__ keys, const uint
   else out = (uint32_t)(p + ((int64_t)1 << l));
   seg_out[e] = out;
 }
+
+// ---- b1, fast form: presorted lists, one stable partition per level -------------------------------------------------
+// The plain order stage above re-sorts all active points by (subtree, coordinate rank) at every level: ceil(log2 N)
+// radix sorts of 64-bit keys.  Sorting is needed only ONCE per dimension (the sort-based k-d build the paper points
+// to): keep, for every dimension a, the list of active point ids grouped by subtree and sorted by
+// (coordinate a, user id) inside each subtree.  At level l the list of the split dimension l mod d names every
+// subtree's median by POSITION (offset = size of its left subtree, known in closed form for the left-balanced tree in
+// bit-reversed numbering, R-2 / PAPER.md:39-41), which gives every point its side; then each list is split
+// stably.  In the bit-reversed numbering the left child of subtree (l, p) is (l + 1, p) and the right child
+// (l + 1, p + 2^l), so the level-(l + 1) list is [all left parts, in subtree order][all right parts, in
+// subtree order]: the per-subtree split IS one global stable three-way partition (left / right / retired median) of the
+// whole list, a single-pass cub::DevicePartition::If.  Order and ties are those of the plain stage (ranks ARE positions
+// in these lists), hence of the oracle, bit for bit.
+__host__ __device__ inline int64_t segment_of(const TreeShape& s, int l, int64_t e, int64_t* q) {
+  // position e of a level-l list -> subtree p (bit-reversed position) and offset q inside it: the first r subtrees
+  // hold base + 1 points, the others base (subtree_prefix inverted)
+  const int64_t step = (int64_t)1 << l;
+  const int64_t full = l < s.lam ? (((int64_t)1 << (s.lam - l)) - 1) : 0;
+  const int64_t base = full + (s.mlast >> l), r = s.mlast & (step - 1);
+  // everything is below 2^31 (n < 2^31): 32-bit divisions
+  if (e < r * (base + 1)) { const uint32_t p = (uint32_t)e / (uint32_t)(base + 1); *q = e - (int64_t)p * (base + 1); return p; }
+  const int64_t e2 = e - r * (base + 1);
+  const uint32_t p2 = (uint32_t)e2 / (uint32_t)base;
+  *q = e2 - (int64_t)p2 * base;
+  return r + p2;
+}
+
+// split dimension's list: side of every active point (0 left, 1 right, 2 = it is node (l, p) and retires)
+__global__ void level_classify_kernel(const uint32_t* __restrict__ lst, int64_t m, int l, TreeShape shape,
+                                      unsigned char* __restrict__ side, uint32_t* __restrict__ perm_tree) {
+  const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (e >= m) return;
+  int64_t q;
+  const int64_t p = segment_of(shape, l, e, &q);
+  const int64_t sl = subtree_size(shape, l + 1, p);
+  const uint32_t id = lst[e];
+  unsigned char c = q < sl ? 0 : (q == sl ? 2 : 1);
+  side[id] = c;
+  if (c == 2) perm_tree[(((int64_t)1 << l) - 1) + p] = id;
+}
+
+// selectors of the three-way stable partition (cub::DevicePartition::If): the id's side
+struct SideIs {
+  const unsigned char* side;
+  unsigned char want;
+  __device__ __forceinline__ bool operator()(const uint32_t& id) const { return side[id] == want; }
+};
 
 template <typename T>
 __global__ void gather_points_kernel(const T* __restrict__ x_src, const uint32_t* __restrict__ idx, int64_t n, int d,
@@ -572,6 +621,7 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
 
   // ---- b1: order -------------------------------------------------------------------------------------
   using CoordKey = typename std::conditional<sizeof(T) == 4, uint32_t, uint64_t>::type;
+  const bool plain_order = (flags & GP_BUILD_PLAIN_ORDER) != 0;
   for (int dim = 0; dim < d; ++dim) {
     CoordKey* ck_a = (CoordKey*)keys_a;
     CoordKey* ck_b = (CoordKey*)keys_b;
@@ -580,10 +630,44 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     cub::DoubleBuffer<CoordKey> kb(ck_a, ck_b);
     cub::DoubleBuffer<uint32_t> vb(vals_a, vals_b);
     GP_OK_OR_RETURN(sort_pairs<CoordKey>(tmp, L.cub_bytes, kb, vb, n, 0, (int)sizeof(CoordKey) * 8, st));
-    scatter_rank_kernel<<<nblk(n), 256, 0, st>>>(vb.Current(), n, rank + (size_t)dim * n);
-    GP_LAUNCH_CHECK();
+    if (plain_order) {
+      scatter_rank_kernel<<<nblk(n), 256, 0, st>>>(vb.Current(), n, rank + (size_t)dim * n);
+      GP_LAUNCH_CHECK();
+    } else {   // the sorted ids ARE the level-0 list of this dimension
+      GP_CUDA_OK(cudaMemcpyAsync(rank + (size_t)dim * n, vb.Current(), (size_t)n * 4, cudaMemcpyDeviceToDevice, st));
+    }
   }
   const TreeShape shape = tree_shape(n);
+  if (!plain_order) {
+    // lists: A in the rank region, B over keys_a + keys_b (contiguous: d * 4 n <= 16 n bytes)
+    if (L.keys_b != L.keys_a + align_up((size_t)n * 8, 256) || L.vals_b != L.vals_a + align_up((size_t)n * 4, 256))
+      return GP_ERR_WORKSPACE;
+    uint32_t* la = rank;
+    uint32_t* lb = (uint32_t*)keys_a;
+    uint32_t* retired = vals_a;                  // where the partition drops the 2^l medians of a level (unused)
+    int* n_sel = (int*)&ctrl->pad[0];            // its two counters (unused)
+    unsigned char* side = (unsigned char*)seg;
+    int64_t m = n;
+    for (int l = 0; l <= shape.lam; ++l) {
+      level_classify_kernel<<<nblk(m), 256, 0, st>>>(la + (size_t)(l % d) * n, m, l, shape, side, perm_tree);
+      GP_LAUNCH_CHECK();
+      if (l == shape.lam) break;                   // the last level: every remaining point is a node
+      const int64_t n_left = subtree_prefix(shape, l + 1, (int64_t)1 << l);   // points in subtrees (l + 1, 0 .. 2^l - 1)
+      for (int a = 0; a < d; ++a) {
+        const uint32_t* in = la + (size_t)a * n;
+        uint32_t* out = lb + (size_t)a * n;
+        size_t need = 0;
+        GP_CUDA_OK(cub::DevicePartition::If(nullptr, need, in, out, out + n_left, retired, n_sel, (int)m, SideIs{side, 0},
+                                            SideIs{side, 1}, st));
+        if (need > L.cub_bytes) return GP_ERR_WORKSPACE;
+        GP_CUDA_OK(cub::DevicePartition::If(tmp, need, in, out, out + n_left, retired, n_sel, (int)m, SideIs{side, 0},
+                                            SideIs{side, 1}, st));
+        count_launch(2);
+      }
+      uint32_t* t_ = la; la = lb; lb = t_;
+      m -= (int64_t)1 << l;
+    }
+  } else {
   int rank_bits = 1;
   while (((int64_t)1 << rank_bits) < n) ++rank_bits;
   {
@@ -604,6 +688,7 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
       GP_LAUNCH_CHECK();
       m_sort = m_active;
     }
+  }
   }
   gather_points_kernel<T><<<nblk(n), 256, 0, st>>>(x_user, perm_tree, n, d, x_tree);
   GP_LAUNCH_CHECK();

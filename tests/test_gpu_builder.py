@@ -114,19 +114,25 @@ def test_builder_large_sampled_rows(gp, orc):
 
 
 @pytest.mark.parametrize("n,d,k,dtype", [(20000, 3, 16, "f32"), (20000, 2, 32, "f32"), (9000, 1, 5, "f64"),
-                                         (12000, 3, 64, "f32"), (7000, 2, 3, "f64"), (30000, 3, 100, "f32")])
-def test_builder_knn_paths_agree_row_for_row(gp, orc, n, d, k, dtype):
-    """The shared-memory kNN walk (default) and the plain one (GP_BUILD_PLAIN_KNN) give the same rows in the same
-    (nearest first, ties by tree index) order, and that order is the oracle's."""
+                                         (12000, 3, 64, "f32"), (7000, 2, 3, "f64"), (30000, 3, 100, "f32"),
+                                         (5000, 4, 6, "f32"), (65537, 3, 8, "f64"), (131, 2, 4, "f32")])
+def test_builder_fast_and_plain_stages_agree_row_for_row(gp, orc, n, d, k, dtype):
+    """Default stages (presorted lists split by one stable partition per level; shared-memory kNN walk) against the
+    plain ones (GP_BUILD_PLAIN_ORDER: a radix sort per level; GP_BUILD_PLAIN_KNN: local-memory walk): same tree order,
+    same rows in the same (nearest first, ties by tree index) order, same depths - and that is the oracle's graph."""
     rng = np.random.default_rng(1000 + k)
     x = rng.standard_normal((n, d)).astype(np.float32 if dtype == "f32" else np.float64)
-    x[50:90] = x[10:50]                                       # exact duplicates: ties in d^2
-    n0 = 128
+    x[50:90] = x[10:50]                                       # exact duplicates: ties in d^2 and in every coordinate
+    x[:, 0] = np.round(x[:, 0] * 8) / 8                       # many equal coordinates in the first split dimension
+    n0 = 128 if n > 128 else 64
     fast = build_gpu(gp, x, k, n0, 0)
-    plain = build_gpu(gp, x, k, n0, gp.GP_BUILD_PLAIN_KNN)
-    assert np.array_equal(fast.perm.cpu().numpy(), plain.perm.cpu().numpy())
-    assert np.array_equal(fast.nbr.cpu().numpy(), plain.nbr.cpu().numpy())
-    assert np.array_equal(fast.depth.cpu().numpy(), plain.depth.cpu().numpy())
-    if k <= 64:
+    for flags in (gp.GP_BUILD_PLAIN_KNN, gp.GP_BUILD_PLAIN_ORDER, gp.GP_BUILD_PLAIN_KNN | gp.GP_BUILD_PLAIN_ORDER):
+        plain = build_gpu(gp, x, k, n0, flags)
+        assert np.array_equal(fast.perm.cpu().numpy(), plain.perm.cpu().numpy())
+        assert np.array_equal(fast.nbr.cpu().numpy(), plain.nbr.cpu().numpy())
+        assert np.array_equal(fast.depth.cpu().numpy(), plain.depth.cpu().numpy())
+        assert np.array_equal(fast.batch_off, plain.batch_off)
+    if k <= 64 and n <= 30000:
         ref = orc.build_graph(x.astype(np.float64), k, n0)
+        assert np.array_equal(fast.perm.cpu().numpy(), ref.perm)
         assert np.array_equal(fast.nbr.cpu().numpy(), ref.nbr)
