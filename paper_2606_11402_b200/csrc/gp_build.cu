@@ -281,11 +281,11 @@ knn_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int d, int k, int64_t
 // Same walk as the plain kernel (pop, prune against the largest plane distance met on the way, visit, descend to the
 // near child, park the far child), restructured after its profile (N = 2^24, config 3: 358 GB of DRAM traffic from the
 // 830 bytes of local memory per thread): everything indexed at run time lives in SHARED memory, [slot][thread] so that
-// a warp's accesses never conflict whatever slots its lanes are at - the stack ({node, bound rounded DOWN to fp32},
-// at most one parked sibling per level) and the k best (d^2, index) pairs as a max-heap whose root is the current
+// a warp's accesses never conflict whatever slots its lanes are at - the stack (one fp32 bound, rounded DOWN, per
+// level: see the kernel) and the k best (d^2, index) pairs as a max-heap whose root is the current
 // k-th best, so accepting a candidate is one replace-root + sift-down (log2 k levels) instead of a rescan of all k.
 // Result identical to the plain kernel, bit for bit (tests/test_gpu_builder.py).  Measured and dropped (DESIGN.md
-// section 7): the stack-FREE traversal the paper points to (ref. Wald 2022b) with the list in registers,
+// section 6.4): the stack-FREE traversal the paper points to (ref. Wald 2022b) with the list in registers,
 // lanes that fetch their next query themselves, and a vote that reconverges the warp every visit.
 // One warp per CTA: a CTA gives its shared memory back when its slowest warp is done, and the queries of different
 // warps differ 2-3x in length on clustered inputs (measured at N = 2^24, kNN stage, CTAs of 128 / 64 / 32 threads:
