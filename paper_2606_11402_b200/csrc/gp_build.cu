@@ -162,25 +162,33 @@ __host__ __device__ inline int64_t segment_of(const TreeShape& s, int l, int64_t
   return r + p2;
 }
 
-// split dimension's list: side of every active point (0 left, 1 right, 2 = it is node (l, p) and retires)
+// Sides are kept as 2 bits per point id (0 left, 1 right, 2 = the point is node (l, p) and retires), 16 ids per word:
+// every list looks the side of its ids up at random, and at N = 2^28 a byte per id (256 MB) no longer fits the L2
+// while 64 MB does.  A thread owns the two bits of its id: it reads them plainly and flips what differs atomically.
+__device__ __forceinline__ uint32_t side_get(const uint32_t* __restrict__ side, uint32_t id) {
+  return (side[id >> 4] >> ((id & 15u) * 2u)) & 3u;
+}
+
+// split dimension's list: side of every active point
 __global__ void level_classify_kernel(const uint32_t* __restrict__ lst, int64_t m, int l, TreeShape shape,
-                                      unsigned char* __restrict__ side, uint32_t* __restrict__ perm_tree) {
+                                      uint32_t* __restrict__ side, uint32_t* __restrict__ perm_tree) {
   const int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= m) return;
   int64_t q;
   const int64_t p = segment_of(shape, l, e, &q);
   const int64_t sl = subtree_size(shape, l + 1, p);
   const uint32_t id = lst[e];
-  unsigned char c = q < sl ? 0 : (q == sl ? 2 : 1);
-  side[id] = c;
-  if (c == 2) perm_tree[(((int64_t)1 << l) - 1) + p] = id;
+  const uint32_t c = q < sl ? 0u : (q == sl ? 2u : 1u);
+  const uint32_t old = side_get(side, id);
+  if (old != c) atomicXor(&side[id >> 4], (old ^ c) << ((id & 15u) * 2u));
+  if (c == 2u) perm_tree[(((int64_t)1 << l) - 1) + p] = id;
 }
 
 // selectors of the three-way stable partition (cub::DevicePartition::If): the id's side
 struct SideIs {
-  const unsigned char* side;
-  unsigned char want;
-  __device__ __forceinline__ bool operator()(const uint32_t& id) const { return side[id] == want; }
+  const uint32_t* side;
+  uint32_t want;
+  __device__ __forceinline__ bool operator()(const uint32_t& id) const { return side_get(side, id) == want; }
 };
 
 template <typename T>
@@ -646,7 +654,8 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     uint32_t* lb = (uint32_t*)keys_a;
     uint32_t* retired = vals_a;                  // where the partition drops the 2^l medians of a level (unused)
     int* n_sel = (int*)&ctrl->pad[0];            // its two counters (unused)
-    unsigned char* side = (unsigned char*)seg;
+    uint32_t* side = seg;                        // 2 bits per id, all "left" to start with
+    GP_CUDA_OK(cudaMemsetAsync(side, 0, ((size_t)n / 16 + 1) * 4, st));
     int64_t m = n;
     for (int l = 0; l <= shape.lam; ++l) {
       level_classify_kernel<<<nblk(m), 256, 0, st>>>(la + (size_t)(l % d) * n, m, l, shape, side, perm_tree);
