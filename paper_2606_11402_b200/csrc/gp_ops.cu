@@ -138,12 +138,13 @@ cond_lg_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const 
 template <typename T, int K, int D, int KIND, int L>
 __global__ void __launch_bounds__(kCondThreads, 3)
 lg_flow_kernel(Rec<T>* rec, const int32_t* __restrict__ nbr, const T* __restrict__ xi, T* __restrict__ out,
-               const longlong4* __restrict__ tab, int nb, int64_t n0, KParams<T> kp, Control* ctrl) {
+               const longlong4* __restrict__ tab, int nb, unsigned long long* ticket, int64_t n0, KParams<T> kp,
+               Control* ctrl) {
   constexpr int PPB = kCondThreads / L;
   constexpr int S = LgShape<T, K, L>::S;
   __shared__ long long s_info[3];
   __shared__ long long s_ticket;
-  if (threadIdx.x == 0) s_ticket = (long long)atomicAdd(&ctrl->ticket, 1ULL);
+  if (threadIdx.x == 0) s_ticket = (long long)atomicAdd(ticket, 1ULL);
   __syncthreads();
   {
     const long long t = s_ticket;
@@ -627,46 +628,78 @@ static gp_status launch_flow(const OpCtx& c, const T* xi, T* v, ForwardPipe* fp)
   return GP_OK;
 }
 
+// Lane-group shapes: the wait-last dataflow body costs about twice the arithmetic of the plain per-point body (the
+// back-substitution runs on group-wide shuffles), so it pays only where the chain of dependent batches is what costs.
+// Stretches of SMALL batches go through lg_flow_kernel (one launch per stretch, own ticket counter), every LARGE batch
+// (at least one wave of CTAs) is one plain launch of cond_lg_kernel.  Measured, config 4 (k = 32, 651 batches):
+// a launch per batch 30.4 ms, dataflow everywhere 37.8 ms, this split 28.3 ms; config 2 fp64: 3.24 / 2.72 / 2.49 ms.
 template <typename T, int K, int D, int L>
 static gp_status launch_lg_flow(const OpCtx& c, const T* xi, T* v) {
   const int nb = c.g->n_batches;
   if (nb <= 0) return GP_OK;
   constexpr int PPB = kCondThreads / L;
-  std::vector<int64_t> tab(4 * (size_t)nb);    // per batch {first chunk, first point, end point, end chunk}
   const int64_t* off = c.g->batch_off;
-  int64_t chunks = 0;
   const int sms = device_sm_count();
   if (sms <= 0) return GP_ERR_CUDA;
   const int64_t resident = (int64_t)sms * 3;   // CTAs the GPU holds at once
-  for (int b = 0; b < nb; ++b) {
-    const int64_t cnt = off[b + 1] - off[b];
-    int64_t rounds = cnt / (2 * resident * PPB);     // keep at least two waves of tickets per batch
-    rounds = rounds < 1 ? 1 : (rounds > 8 ? 8 : rounds);
-    int64_t nc = (cnt + PPB * rounds - 1) / (PPB * rounds);
-    tab[4 * b + 0] = chunks;
-    tab[4 * b + 1] = (rounds << 40) | off[b];
-    tab[4 * b + 2] = off[b + 1];
-    tab[4 * b + 3] = chunks + nc;
-    chunks += nc;
+  const int64_t large = resident * PPB;        // one full wave; measured flat between 1 and 4 waves, worse beyond
+  auto is_big = [&](int q) {
+    if (c.g->flags & GP_FLAG_FLOW_WEIGHTS) return false;
+    return off[q + 1] - off[q] >= large;
+  };
+  struct Stretch { int b, e; bool big; int64_t chunks; };
+  std::vector<Stretch> plan;
+  std::vector<int64_t> tab(4 * (size_t)nb);    // per batch {first chunk, rounds << 40 | first point, end point, end chunk}
+  for (int b = 0; b < nb;) {
+    const bool big = is_big(b);
+    int e = b + 1;
+    if ((int)plan.size() >= kFlowTickets - 1 && !big) e = nb;   // the last ticket counter takes everything that is left
+    else if (!big) while (e < nb && !is_big(e)) ++e;
+    int64_t chunks = 0;
+    if (!big) {
+      for (int q = b; q < e; ++q) {              // chunk numbers restart with every stretch
+        const int64_t cnt = off[q + 1] - off[q];
+        int64_t rounds = cnt / (2 * resident * PPB);   // keep at least two waves of tickets per batch
+        rounds = rounds < 1 ? 1 : (rounds > 8 ? 8 : rounds);
+        const int64_t nc = (cnt + PPB * rounds - 1) / (PPB * rounds);
+        tab[4 * q + 0] = chunks;
+        tab[4 * q + 1] = (rounds << 40) | off[q];
+        tab[4 * q + 2] = off[q + 1];
+        tab[4 * q + 3] = chunks + nc;
+        chunks += nc;
+      }
+      if (chunks > 0x7fffffffLL) return GP_ERR_UNSUPPORTED;
+    }
+    plan.push_back({b, e, big, chunks});
+    b = e;
   }
-  if (chunks <= 0 || chunks > 0x7fffffffLL) return GP_ERR_UNSUPPORTED;
   // pageable source: the runtime stages it before returning, so the vector may die afterwards
   GP_CUDA_OK(cudaMemcpyAsync(c.boff_dev(), tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, c.st));
   KParams<T> kp = make_kparams<T>(*c.kern);
   Rec<T>* rec = (Rec<T>*)c.rec();
-  const longlong4* tab_d = (const longlong4*)c.boff_dev();
-  switch (c.kern->kind) {
-    case GP_KERNEL_SE:
-      lg_flow_kernel<T, K, D, GP_KERNEL_SE, L><<<(unsigned)chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, nb, c.g->n0, kp, c.ctrl());
-      break;
-    case GP_KERNEL_MATERN32:
-      lg_flow_kernel<T, K, D, GP_KERNEL_MATERN32, L><<<(unsigned)chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, nb, c.g->n0, kp, c.ctrl());
-      break;
-    default:
-      lg_flow_kernel<T, K, D, GP_KERNEL_EXP, L><<<(unsigned)chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, nb, c.g->n0, kp, c.ctrl());
-      break;
+  int slot = 0;
+  for (const Stretch& s : plan) {
+    if (s.big) {
+      GP_OK_OR_RETURN((launch_range<T, OPK_FORWARD>(c, true, v, xi, v, off[s.b], off[s.e])));
+      continue;
+    }
+    const longlong4* tab_d = (const longlong4*)c.boff_dev() + s.b;
+    const int cnt = s.e - s.b;
+    unsigned long long* ticket = &c.ctrl()->flow_ticket[slot < kFlowTickets ? slot : kFlowTickets - 1];
+    ++slot;
+    switch (c.kern->kind) {
+      case GP_KERNEL_SE:
+        lg_flow_kernel<T, K, D, GP_KERNEL_SE, L><<<(unsigned)s.chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, cnt, ticket, c.g->n0, kp, c.ctrl());
+        break;
+      case GP_KERNEL_MATERN32:
+        lg_flow_kernel<T, K, D, GP_KERNEL_MATERN32, L><<<(unsigned)s.chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, cnt, ticket, c.g->n0, kp, c.ctrl());
+        break;
+      default:
+        lg_flow_kernel<T, K, D, GP_KERNEL_EXP, L><<<(unsigned)s.chunks, kCondThreads, 0, c.st>>>(rec, c.g->nbr, xi, v, tab_d, cnt, ticket, c.g->n0, kp, c.ctrl());
+        break;
+    }
+    GP_LAUNCH_CHECK();
   }
-  GP_LAUNCH_CHECK();
   return GP_OK;
 }
 
@@ -679,11 +712,9 @@ static gp_status forward_t(const OpCtx& c, const T* xi, T* v) {
     if (std::is_same<TT, T>::value && c.g->k == K && c.g->d == D) flow = true;
     GP_SPEC_TABLE(X)
 #undef X
-    // lane-group shapes: measured, the dataflow launch wins for fp64 k = 16 (config 2: 3.2 -> 2.8 ms) and loses for
-    // fp32 k = 32 (config 4: 30.5 -> 38.5 ms, 651 batches), so k = 32 keeps the launch per batch unless asked
+    // lane-group shapes: dataflow launches for the stretches of small batches, a plain launch per large batch
 #define X(TT, K, D, L) \
-    if (std::is_same<TT, T>::value && c.g->k == K && c.g->d == D && (sizeof(T) == 8 || (c.g->flags & GP_FLAG_FLOW_WEIGHTS))) \
-      flow = true;
+    if (std::is_same<TT, T>::value && c.g->k == K && c.g->d == D) flow = true;
     GP_LG_TABLE(X)
 #undef X
   }
