@@ -102,7 +102,7 @@ cond_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* 
 
 // ---- lane-group kernel: one point per L lanes (k = 32 fp32, k = 16 fp64) -----------------------------------
 template <typename T, int K, int D, int KIND, int L, int OP>
-__global__ void __launch_bounds__(kCondThreads, 3)
+__global__ void __launch_bounds__(kCondThreads, sizeof(T) == 8 ? 4 : 3)
 cond_lg_kernel(Rec<T>* __restrict__ rec, const int32_t* __restrict__ nbr, const T* __restrict__ in, T* __restrict__ out,
                int64_t start, int64_t end, int64_t n0, KParams<T> kp, Control* ctrl) {
   __shared__ double red[32];
