@@ -200,6 +200,16 @@ __global__ void gather_points_kernel(const T* __restrict__ x_src, const uint32_t
   for (int t = 0; t < d; ++t) x_dst[i * d + t] = x_src[s * d + t];
 }
 
+__global__ void pack_points4_kernel(const float* __restrict__ x, int64_t n, int d, float4* __restrict__ x4) {
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+  v.x = x[i * d];
+  if (d >= 2) v.y = x[i * d + 1];
+  if (d >= 3) v.z = x[i * d + 2];
+  x4[i] = v;
+}
+
 // ---- b2: preceding kNN --------------------------------------------------------------------------------
 // canonical squared distance (R-5): double, left-to-right, no FMA contraction
 template <typename T>
@@ -327,10 +337,13 @@ __device__ __forceinline__ void heap_replace_root(double* hd, int32_t* hi, int k
   hi[pos * kKnnThreads] = ni;
 }
 
-template <typename T, int D>
+// x4: for fp32 inputs the tree-ordered coordinates once more as one aligned 16-byte record per point ({x, y, z, 0}), so a
+// node visit is one LDG.128 inside one sector instead of D scalar loads of a 4 D-byte record that straddles two sectors
+// three times out of eight; nullptr for fp64 inputs.
+template <typename T, int D, bool PACK4>
 __global__ void __launch_bounds__(kKnnThreads)
-knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int nlev, int64_t n_threads,
-              int32_t* __restrict__ nbr, float* __restrict__ rad2) {
+knn_sm_kernel(const T* __restrict__ x, const float4* __restrict__ x4, int64_t n, int64_t n0, int k, int nlev,
+              int64_t n_threads, int32_t* __restrict__ nbr, float* __restrict__ rad2) {
   extern __shared__ double knn_smem[];
   double* hd = knn_smem + threadIdx.x;                                                           // [k][kKnnThreads]
   int32_t* hi = reinterpret_cast<int32_t*>(knn_smem + (size_t)k * kKnnThreads) + threadIdx.x;     // [k][kKnnThreads]
@@ -375,12 +388,22 @@ knn_sm_kernel(const T* __restrict__ x, int64_t n, int64_t n0, int k, int nlev, i
       have = true;
     }
     if ((double)bound > wd) { have = false; continue; }
-    const T* xc = x + (int64_t)curr * D;
+    double xn[D];
+    if constexpr (PACK4) {
+      const float4 v = __ldg(x4 + curr);
+      xn[0] = (double)v.x;
+      if (D >= 2) xn[1] = (double)v.y;
+      if (D >= 3) xn[2] = (double)v.z;
+    } else {
+      const T* xc = x + (int64_t)curr * D;
+#pragma unroll
+      for (int a = 0; a < D; ++a) xn[a] = (double)__ldg(xc + a);
+    }
     const int dim = lc % D;
     double acc = 0.0, diff = 0.0;
 #pragma unroll
     for (int a = 0; a < D; ++a) {
-      const double dx = __dsub_rn(xi[a], (double)__ldg(xc + a));
+      const double dx = __dsub_rn(xi[a], xn[a]);
       const double sq = __dmul_rn(dx, dx);
       acc = a == 0 ? sq : __dadd_rn(acc, sq);
       diff = a == dim ? dx : diff;
@@ -712,10 +735,21 @@ static gp_status build_t(const T* x_user, int64_t n, int d, int k, int64_t n0, i
     const int nlev = shape.lam + 2;                // levels 0 .. lam + 1 can be indexed (level 0 is never parked)
     const size_t sm_bytes = (size_t)kKnnThreads * (12 * (size_t)k + 4 * (size_t)nlev);
     if (!plain && d <= 3 && sm_bytes <= 200 * 1024) {
-#define GP_KNN_SM(DD) { \
-      GP_CUDA_OK(cudaFuncSetAttribute(knn_sm_kernel<T, DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); \
-      knn_sm_kernel<T, DD><<<nblk(n_threads, kKnnThreads), kKnnThreads, sm_bytes, st>>>(x_tree, n, n0, k, nlev, n_threads, nbr_tree, rad2); }
+      // fp32: the order stage's key buffers (16 n bytes, contiguous, checked there) are dead until the depth sort
+      const float4* x4 = nullptr;
+      // (only once the coordinates no longer fit the L2: measured 975 -> 881 ms at N = 2^28, 209 -> 202 ms at 2^26,
+      // and 61 -> 62 ms at 2^24, where the extra pass is all it adds)
+      if (sizeof(T) == 4 && (size_t)n * d * 4 > ((size_t)96 << 20) && L.keys_b == L.keys_a + align_up((size_t)n * 8, 256)) {
+        pack_points4_kernel<<<nblk(n), 256, 0, st>>>((const float*)x_tree, n, d, (float4*)keys_a);
+        GP_LAUNCH_CHECK();
+        x4 = (const float4*)keys_a;
+      }
+#define GP_KNN_SM2(DD, P4) { \
+      GP_CUDA_OK(cudaFuncSetAttribute(knn_sm_kernel<T, DD, P4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024)); \
+      knn_sm_kernel<T, DD, P4><<<nblk(n_threads, kKnnThreads), kKnnThreads, sm_bytes, st>>>(x_tree, x4, n, n0, k, nlev, n_threads, nbr_tree, rad2); }
+#define GP_KNN_SM(DD) { if (x4) GP_KNN_SM2(DD, true) else GP_KNN_SM2(DD, false) }
       if (d == 1) GP_KNN_SM(1) else if (d == 2) GP_KNN_SM(2) else GP_KNN_SM(3)
+#undef GP_KNN_SM2
 #undef GP_KNN_SM
     }
     else if (k <= 16) knn_kernel<T, 16><<<nblk(n_threads, 128), 128, 0, st>>>(x_tree, n, n0, d, k, n_threads, nbr_tree, rad2, ovf);
