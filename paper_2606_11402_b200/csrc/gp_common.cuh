@@ -115,6 +115,27 @@ template <> struct Math<float> {
     return t * ln2 * ex2(-t);                                               // rho * r/ell
   }
 };
+// e^-a for a >= 0 in double, branch-free, coefficients in constant memory (operands of the DFMAs themselves).  The
+// library exp costs the fp64 lane-group kernels a quarter of their instructions in constants moved through uniform
+// registers at every call site and in the branches around its special cases (profiles/r2_ncu_full.md).  Cody-Waite
+// reduction a = n ln2 + r', |r'| <= ln2 / 2, degree-13 Taylor polynomial of e^-r' (truncation 6e-18), scaling by the
+// exponent field; a > 700 gives 0.  Error about 1 ulp, as the library's.
+__constant__ double kExpNegC[14] = {1.0, 1.0, 0.5, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
+                                    1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
+__device__ __forceinline__ double exp_neg(double a) {
+  const double shift = 6755399441055744.0;                      // 1.5 * 2^52: round to nearest integer in the low bits
+  const double t = ::fma(a, 1.4426950408889634074, shift);
+  const int n = __double2loint(t);
+  const double nf = t - shift;
+  double r = ::fma(nf, 6.93147180369123816490e-01, -a);         // r = n ln2 - a = -r'
+  r = ::fma(nf, 1.90821492927058770002e-10, r);
+  double p = kExpNegC[13];
+#pragma unroll
+  for (int q = 12; q >= 0; --q) p = ::fma(p, r, kExpNegC[q]);
+  const double scale = __hiloint2double((1023 - n) << 20, 0);   // 2^-n, n <= 1010 where it is used
+  return a > 700.0 ? 0.0 : p * scale;
+}
+
 template <> struct Math<double> {
   static __device__ __forceinline__ double rsqrt(double x) { return 1.0 / ::sqrt(x); }
   static __device__ __forceinline__ double sqrt(double x) { return ::sqrt(x); }
@@ -122,10 +143,10 @@ template <> struct Math<double> {
   static __device__ __forceinline__ double log(double x) { return ::log(x); }
   static __device__ __forceinline__ double fmin(double a, double b) { return ::fmin(a, b); }
   template <int KIND> static __device__ __forceinline__ double rho_from_q(double q) {
-    if (KIND == GP_KERNEL_SE) return ::exp(-q);
+    if (KIND == GP_KERNEL_SE) return exp_neg(q);
     double a = ::sqrt(q);
-    if (KIND == GP_KERNEL_MATERN32) return (1.0 + a) * ::exp(-a);
-    return ::exp(-a);
+    if (KIND == GP_KERNEL_MATERN32) return (1.0 + a) * exp_neg(a);
+    return exp_neg(a);
   }
   template <int KIND> static __device__ __forceinline__ double drho_from_q(double q) {
     if (KIND == GP_KERNEL_SE) return 2.0 * q * ::exp(-q);
