@@ -220,12 +220,12 @@ constexpr int kScatterThreads = 256;
 template <int K>
 __global__ void __launch_bounds__(kScatterThreads, 4)
 vjp_scatter_kernel(const int32_t* __restrict__ nbr, const float* __restrict__ wbuf, const float4* __restrict__ sab,
-                   float* gbar, float* __restrict__ xibar, const longlong4* __restrict__ tab, int L, int64_t n0,
-                   int64_t n, float sigma, Control* ctrl) {
+                   float* gbar, float* __restrict__ xibar, const longlong4* __restrict__ tab, int L,
+                   unsigned long long* ticket, int64_t n0, int64_t n, float sigma, Control* ctrl) {
   __shared__ double red[32];
   __shared__ long long s_info[3];
   __shared__ long long s_ticket;
-  if (threadIdx.x == 0) s_ticket = (long long)atomicAdd(&ctrl->ticket, 1ULL);
+  if (threadIdx.x == 0) s_ticket = (long long)atomicAdd(ticket, 1ULL);
   __syncthreads();
   {
     const long long t = s_ticket;
@@ -560,14 +560,23 @@ static gp_status launch_vjp_geom(const OpCtx& c, const float* xi, int64_t first,
 
 // the reverse sweep proper over all batches (ticketed dataflow, last batch first)
 template <int K>
-static gp_status launch_vjp_scatter(const OpCtx& c, float* gbar, float* xibar) {
+static gp_status launch_vjp_scatter(const OpCtx& c, float* gbar, float* xibar, EventBag* bag = nullptr) {
   const int L = c.g->n_batches;
   const int64_t cnt = c.g->n - c.g->n0;
   if (L <= 0 || cnt <= 0) return GP_OK;
-  // device table, one entry per batch in REVERSE order: {first chunk, first point, end point, end chunk}
+  // Host-buffer variant (bag != nullptr): the reverse sweep is cut into up to kScatterParts launches at batch
+  // boundaries, each with its own ticket counter (`done` keeps counting across them), and the xi_bar of a part goes
+  // home on the copy-out stream while the next part runs.  Otherwise one launch.
+  constexpr int kScatterParts = 4;
+  const int parts = bag ? kScatterParts : 1;
+  // device table, one entry per batch in REVERSE order: {first chunk, first point, end point, end chunk}; chunk
+  // numbers restart with every part
   std::vector<int64_t> tab(4 * (size_t)L);
   const int64_t* off = c.g->batch_off;
-  int64_t chunks = 0;
+  struct Part { int r0, r1; int64_t chunks; };
+  std::vector<Part> plan;
+  int64_t chunks = 0, pts = 0;
+  int r0 = 0;
   for (int rb = 0; rb < L; ++rb) {
     int b = L - 1 - rb;
     int64_t nc = (off[b + 1] - off[b] + kScatterThreads - 1) / kScatterThreads;
@@ -576,16 +585,34 @@ static gp_status launch_vjp_scatter(const OpCtx& c, float* gbar, float* xibar) {
     tab[4 * rb + 2] = off[b + 1];
     tab[4 * rb + 3] = chunks + nc;
     chunks += nc;
+    pts += off[b + 1] - off[b];
+    const bool last = rb == L - 1;
+    if (last || ((int)plan.size() < parts - 1 && pts >= cnt * ((int64_t)plan.size() + 1) / parts)) {
+      if (chunks > 0x7fffffffLL) return GP_ERR_UNSUPPORTED;
+      plan.push_back({r0, rb + 1, chunks});
+      r0 = rb + 1;
+      chunks = 0;
+    }
   }
-  if (chunks <= 0 || chunks > 0x7fffffffLL) return GP_ERR_UNSUPPORTED;
   // pageable source: the runtime stages it before returning, so the vector may die afterwards
   GP_CUDA_OK(cudaMemcpyAsync(c.boff_dev(), tab.data(), tab.size() * sizeof(int64_t), cudaMemcpyHostToDevice, c.st));
-  const longlong4* tab_d = (const longlong4*)c.boff_dev();
   float* wbuf = c.wbuf();
   float4* sab = reinterpret_cast<float4*>(wbuf + (size_t)cnt * K);
-  vjp_scatter_kernel<K><<<(unsigned)chunks, kScatterThreads, 0, c.st>>>(c.g->nbr, wbuf, sab, gbar, xibar, tab_d, L, c.g->n0,
-                                                                      c.g->n, (float)c.kern->sigma, c.ctrl());
-  GP_LAUNCH_CHECK();
+  int slot = 0;
+  for (const Part& p : plan) {
+    if (p.chunks <= 0) continue;
+    const longlong4* tab_d = (const longlong4*)c.boff_dev() + p.r0;
+    unsigned long long* ticket = plan.size() == 1 ? &c.ctrl()->ticket : &c.ctrl()->flow_ticket[slot++];
+    vjp_scatter_kernel<K><<<(unsigned)p.chunks, kScatterThreads, 0, c.st>>>(c.g->nbr, wbuf, sab, gbar, xibar, tab_d, p.r1 - p.r0,
+                                                                          ticket, c.g->n0, c.g->n, (float)c.kern->sigma, c.ctrl());
+    GP_LAUNCH_CHECK();
+    if (bag) {                                 // points of reverse batches [r0, r1) = graph positions [lo, hi)
+      const int64_t lo = off[L - p.r1], hi = off[L - p.r0];
+      GP_OK_OR_RETURN(stream_after(*bag, c.io->cout, c.st));
+      GP_CUDA_OK(cudaMemcpyAsync((float*)c.io->out_host + lo, xibar + lo, (size_t)(hi - lo) * sizeof(float),
+                                 cudaMemcpyDeviceToHost, c.io->cout));
+    }
+  }
   return GP_OK;
 }
 
@@ -610,10 +637,11 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
   // host-buffer variant: v and xi arrive range by range beside the geometry kernel (a point reads only points before
   // it), then v_bar; xi_bar goes home at the end
   EventBag bag;
-  const int chunks = (c.io && flow) ? 4 : 1;
-  int64_t cut[5];
+  constexpr int kVjpChunks = 8;
+  const int chunks = (c.io && flow) ? kVjpChunks : 1;
+  int64_t cut[kVjpChunks + 1];
   for (int q = 0; q <= chunks; ++q) cut[q] = q == 0 ? 0 : (q == chunks ? n : n0 + (n - n0) * q / chunks);
-  cudaEvent_t arrived[4] = {}, vbar_arrived = nullptr;
+  cudaEvent_t arrived[kVjpChunks] = {}, vbar_arrived = nullptr;
   if (c.io) {
     GP_OK_OR_RETURN(stream_after(bag, c.io->cin, c.st));
     for (int q = 0; q < chunks; ++q) {
@@ -653,8 +681,8 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
       }
       if (c.io) GP_CUDA_OK(cudaStreamWaitEvent(c.st, vbar_arrived, 0));
       GP_CUDA_OK(cudaMemcpyAsync(gbar, vbar, (size_t)n * sizeof(T), cudaMemcpyDeviceToDevice, c.st));
-      if (c.g->k == 8) GP_OK_OR_RETURN((launch_vjp_scatter<8>(c, gbar, xibar)));
-      else GP_OK_OR_RETURN((launch_vjp_scatter<16>(c, gbar, xibar)));
+      if (c.g->k == 8) GP_OK_OR_RETURN((launch_vjp_scatter<8>(c, gbar, xibar, c.io ? &bag : nullptr)));
+      else GP_OK_OR_RETURN((launch_vjp_scatter<16>(c, gbar, xibar, c.io ? &bag : nullptr)));
     }
   } else {
     if (c.io) {
@@ -672,7 +700,12 @@ static gp_status vjp_t(const OpCtx& c, const T* xi, const T* v, const T* vbar, T
   if (n0 > 0) GP_OK_OR_RETURN(head_vjp(c, xi, gbar, xibar, &c.ctrl()->acc[3]));
   finalize_grad_kernel<<<1, 32, 0, c.st>>>(c.ctrl(), 3, 4, 1.0 / c.kern->ell, thetabar);
   GP_LAUNCH_CHECK();
-  if (c.io) GP_CUDA_OK(cudaMemcpyAsync(c.io->out_host, xibar, (size_t)n * sizeof(T), cudaMemcpyDeviceToHost, c.st));
+  if (c.io) {
+    // the dataflow path has sent xi_bar[n0:] home part by part already: only the head's xi_bar is left
+    const int64_t cnt_out = (flow && n > n0) ? n0 : n;
+    GP_CUDA_OK(cudaMemcpyAsync(c.io->out_host, xibar, (size_t)cnt_out * sizeof(T), cudaMemcpyDeviceToHost, c.st));
+    GP_OK_OR_RETURN(stream_after(bag, c.st, c.io->cout));   // the caller's stream ends when all of xi_bar is on the host
+  }
   return GP_OK;
 }
 
