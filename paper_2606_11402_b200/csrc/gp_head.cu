@@ -125,6 +125,12 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
   __shared__ __align__(16) double Pc[NB][64 + 2];
   const int tid = threadIdx.x, lane = tid & 31;
   const int G = gridDim.x;
+  // LOOK-AHEAD (G >= 2): the last CTA takes no tiles; during phase 2 of panel p it updates the NEXT 32 x 32 diagonal
+  // block, factors it and writes the factor to A, so that in phase 1 of panel p + 1 every CTA just reads the factored
+  // block instead of all of them repeating its 32-step pivot chain on the critical path (profiles/r2_head_samples.md:
+  // 27 % of the warp samples sat in the barrier behind that chain).  The tile owners leave that block alone.
+  const bool la = G >= 2;
+  const int GT = la ? G - 1 : G;                      // CTAs that take tiles
   for (int j0 = 0; j0 < n0; j0 += NB) {
     const int nb = min(NB, n0 - j0);
     const int j1 = j0 + nb;
@@ -135,16 +141,26 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
     const int warp = tid >> 5, nwarp = blockDim.x >> 5;
     const int first_row = j1 + (int)blockIdx.x * nwarp + warp;
     if ((int)blockIdx.x * nwarp < below || blockIdx.x == 0) {
-      if (tid < 32) {
-        double a[NB];
+      if (!la || j0 == 0) {
+        if (tid < 32) {
+          double a[NB];
 #pragma unroll
-        for (int c = 0; c < NB; ++c)
-          a[c] = (lane < nb && c <= lane && c < nb) ? A[(size_t)(j0 + lane) * n0 + j0 + c] : (c == lane ? 1.0 : 0.0);
-        bool bad = false;
-        DiagStep<0>::run(a, lane, invd, colbuf, bad);
-        if (bad && blockIdx.x == 0 && lane == 0) atomicAdd(&ctrl->n_bad, 1ULL);
+          for (int c = 0; c < NB; ++c)
+            a[c] = (lane < nb && c <= lane && c < nb) ? A[(size_t)(j0 + lane) * n0 + j0 + c] : (c == lane ? 1.0 : 0.0);
+          bool bad = false;
+          DiagStep<0>::run(a, lane, invd, colbuf, bad);
+          if (bad && blockIdx.x == 0 && lane == 0) atomicAdd(&ctrl->n_bad, 1ULL);
 #pragma unroll
-        for (int c = 0; c < NB; ++c) Ds[lane][c] = c <= lane ? a[c] : 0.0;
+          for (int c = 0; c < NB; ++c) Ds[lane][c] = c <= lane ? a[c] : 0.0;
+        }
+      } else {
+        // the factored block is in A already (look-ahead CTA, previous phase 2)
+        for (int e = tid; e < NB * NB; e += blockDim.x) {
+          const int r = e / NB, cc = e % NB;
+          Ds[r][cc] = (r < nb && cc <= r) ? A[(size_t)(j0 + r) * n0 + j0 + cc] : (r == cc ? 1.0 : 0.0);
+        }
+        __syncthreads();
+        if (tid < NB) invd[tid] = 1.0 / Ds[tid][tid];
       }
       __syncthreads();
       for (int r = first_row; r < rows_total; r += G * nwarp) {
@@ -161,19 +177,55 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
     }
     grid.sync();
     // ---- phase 2 --------------------------------------------------------------------------------------
-    // CTA 0 writes the factored diagonal block back only now: during phase 1 the other CTAs were still reading the
-    // unfactored block from A (every CTA factors its own copy), and nothing in this kernel reads it again.
-    if (blockIdx.x == 0) {
+    // Without look-ahead (and for the first panel) CTA 0 writes the factored diagonal block back only now: during phase 1
+    // the other CTAs were still reading the unfactored block from A (every CTA factors its own copy), and nothing in
+    // this kernel reads it again.
+    if (blockIdx.x == 0 && (!la || j0 == 0)) {
       for (int e = tid; e < NB * NB; e += blockDim.x) {
         const int r = e / NB, cc = e % NB;
         if (r < nb && cc <= r) A[(size_t)(j0 + r) * n0 + j0 + cc] = Ds[r][cc];
       }
     }
     const int cols = n0 - j1;
-    if (cols > 0) {
+    if (cols > 0 && la && blockIdx.x == G - 1) {
+      // next diagonal block: D = A[j1 : j1 + nb2][j1 : j1 + nb2] - P P^T with P = the panel rows just solved, then factor
+      const int nb2 = min(NB, n0 - j1);
+      __syncthreads();
+      for (int e = tid; e < NB * NB; e += blockDim.x) {
+        const int row = e / NB, tt = e % NB;
+        Pr[tt][row] = (row < nb2 && tt < nb) ? A[(size_t)(j1 + row) * n0 + j0 + tt] : 0.0;
+      }
+      __syncthreads();
+      for (int e = tid; e < NB * NB; e += blockDim.x) {
+        const int r = e / NB, cc = e % NB;
+        double v = r == cc ? 1.0 : 0.0;                // padding of a short last block: identity
+        if (r < nb2 && cc <= r) {
+          double acc = 0.0;
+#pragma unroll 8
+          for (int tt = 0; tt < NB; ++tt) acc = fma(Pr[tt][r], Pr[tt][cc], acc);
+          v = A[(size_t)(j1 + r) * n0 + j1 + cc] - acc;
+        } else if (cc > r) {
+          v = 0.0;
+        }
+        Ds[r][cc] = v;
+      }
+      __syncthreads();
+      if (tid < 32) {
+        double a[NB];
+#pragma unroll
+        for (int c = 0; c < NB; ++c) a[c] = Ds[lane][c];
+        bool bad = false;
+        DiagStep<0>::run(a, lane, invd, colbuf, bad);
+        if (bad && lane == 0) atomicAdd(&ctrl->n_bad, 1ULL);
+#pragma unroll
+        for (int c = 0; c < NB; ++c)
+          if (lane < nb2 && c <= lane) A[(size_t)(j1 + lane) * n0 + j1 + c] = a[c];
+      }
+    } else if (cols > 0) {
       const int ntc = (cols + 63) / 64, ntr = (below + 63) / 64;
+      const int nb2t = min(NB, n0 - j1);             // size of the next diagonal block
       // valid tiles only: for a row tile inside the square part, column tiles up to the diagonal
-      for (int t = blockIdx.x;; t += G) {
+      for (int t = blockIdx.x;; t += GT) {
         // map t to the t-th valid tile: rows tr < ntc are triangular (tr + 1 tiles), the rest are full
         int tr, tc;
         const int tri_tiles = ntc * (ntc + 1) / 2;
@@ -225,6 +277,8 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
           for (int b_ = 0; b_ < 4; ++b_) {
             int cidx = c0 + tx * 4 + b_;
             if (cidx >= n0 || (r < n0 && cidx > r)) continue;
+            if (la && r < j1 + nb2t) continue;         // the next diagonal block (rows j1 .. j1 + nb2t - 1, all their
+                                                       // columns >= j1) belongs to the look-ahead CTA
             A[(size_t)r * n0 + cidx] -= acc[a_][b_];
           }
         }
