@@ -115,8 +115,12 @@ template <> struct DiagStep<NB> {
   static __device__ __forceinline__ void run(double (&)[NB], int, double*, double*, bool&) {}
 };
 
-__global__ void __launch_bounds__(256)
-head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) {
+// Two entry points (below): head_chol_kernel_128 is capped at 128 registers (a few spills) - beside the VJP's geometry pass,
+// 255 registers x 128 threads, one geometry CTA must still fit on an SM that holds a head CTA, or the geometry pass loses
+// those SMs (VJP 8.27 against 8.38 ms); head_chol_kernel is unconstrained (142 registers, no spill).  An explicit minimum
+// of one CTA per SM made the compiler take 255 registers, and then no bulk CTA fits beside the head at all.
+static __device__ __forceinline__ void head_chol_body(double* __restrict__ A, int n0, int rows_total, int lookahead,
+                                                      Control* ctrl) {
   cg::grid_group grid = cg::this_grid();
   __shared__ double Ds[NB][NB + 1];
   __shared__ double invd[NB];
@@ -129,7 +133,7 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
   // block, factors it and writes the factor to A, so that in phase 1 of panel p + 1 every CTA just reads the factored
   // block instead of all of them repeating its 32-step pivot chain on the critical path (profiles/r2_head_samples.md:
   // 27 % of the warp samples sat in the barrier behind that chain).  The tile owners leave that block alone.
-  const bool la = G >= 2;
+  const bool la = lookahead && G >= 2;
   const int GT = la ? G - 1 : G;                      // CTAs that take tiles
   for (int j0 = 0; j0 < n0; j0 += NB) {
     const int nb = min(NB, n0 - j0);
@@ -288,6 +292,15 @@ head_chol_kernel(double* __restrict__ A, int n0, int rows_total, Control* ctrl) 
   }
 }
 
+__global__ void __launch_bounds__(256) head_chol_kernel(double* __restrict__ A, int n0, int rows_total, int lookahead,
+                                                        Control* ctrl) {
+  head_chol_body(A, n0, rows_total, lookahead, ctrl);
+}
+__global__ void __launch_bounds__(256, 2) head_chol_kernel_128(double* __restrict__ A, int n0, int rows_total,
+                                                               int lookahead, Control* ctrl) {
+  head_chol_body(A, n0, rows_total, lookahead, ctrl);
+}
+
 static gp_status head_build(const OpCtx& c) {
   const int n0 = (int)c.g->n0;
   KParams<double> kp = make_kparams<double>(*c.kern);
@@ -308,7 +321,8 @@ static gp_status head_chol(const OpCtx& c, int n_carried, bool overlapped) {
   if (grid_ctas <= 0) return GP_ERR_CUDA;
   int n0_arg = n0;
   Control* ctrl = c.ctrl();
-  void* args[] = {(void*)&A, (void*)&n0_arg, (void*)&rows_total, (void*)&ctrl};
+  int lookahead = 1;
+  void* args[] = {(void*)&A, (void*)&n0_arg, (void*)&rows_total, (void*)&lookahead, (void*)&ctrl};
   int ctas = grid_ctas;
   // beside a LONG bulk kernel the head takes a quarter of the SMs (more when many rows are carried) and is hidden;
   // beside a short one (config 2: 2^20 points, 0.2 ms of bulk work) it is the critical path and takes every SM
@@ -316,7 +330,8 @@ static gp_status head_chol(const OpCtx& c, int n_carried, bool overlapped) {
     ctas = n_carried > n0 ? grid_ctas / 2 : grid_ctas / 4;
     if (ctas < 1) ctas = 1;
   }
-  GP_CUDA_OK(cudaLaunchCooperativeKernel((const void*)head_chol_kernel, dim3(ctas), dim3(256), args, 0, c.st));
+  const void* fn = n_carried > 1 ? (const void*)head_chol_kernel_128 : (const void*)head_chol_kernel;
+  GP_CUDA_OK(cudaLaunchCooperativeKernel(fn, dim3(ctas), dim3(256), args, 0, c.st));
   GP_LAUNCH_CHECK();
   return GP_OK;
 }
